@@ -1,0 +1,382 @@
+"""Pins of the FP64 oracle against what the paper and the mathematics fix (no GPU).
+
+P1..P13 follow SURVEY.md section 8(c).  The paper prints no numeric worked example, so the
+pins are closed forms (tests/golden/closed_forms.txt), finite differences, invariants, special
+cases and brute force, chosen so that a dropped term, a wrong sign/index or a transposed operand
+in oracle/mop_oracle.c fails at least one of them.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2501_11962_b200 import workloads as W
+from tests import helpers as H
+
+KE = 138.935458
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")) as f:
+    for line in f:
+        if not line.startswith("#"):
+            k, v = line.split()
+            GOLD[k] = float(v)
+
+
+# ---------------------------------------------------------------- P1 / P2 closed forms
+@pytest.mark.parametrize("r", [0.30, 0.34, 0.40, 0.55, 0.90])
+def test_P1_lj_two_atom_closed_form(oracle, r):
+    """LJ 12-6 energy and force of an isolated pair vs the textbook closed form."""
+    for axis in range(3):
+        s = H.two_atoms(r, axis=axis)
+        o = oracle.OracleSystem(s)
+        for geom in (0, 1):
+            res = oracle.bead(o, s.R1, geom=geom, brute=True)
+            assert res["npairs"] == 1
+            # geom 1 first rounds the coordinates to float32 (relative 6e-8 on r, x13 on the force)
+            tol = 3e-6 if geom == 0 else 1e-4
+            assert res["U"][0] == pytest.approx(GOLD["lj_u_r=%.2f" % r], rel=tol, abs=tol)
+            F = res["F"]
+            # atom 1 sits at +r along `axis`: repulsive force pushes it towards +axis
+            assert F[1, axis] == pytest.approx(GOLD["lj_F_r=%.2f" % r], rel=tol)
+            assert F[0, axis] == pytest.approx(-GOLD["lj_F_r=%.2f" % r], rel=tol)
+            off = [a for a in range(3) if a != axis]
+            assert np.abs(F[:, off]).max() < 1e-9
+
+
+def test_P1_lj_minimum_and_curvature(oracle):
+    rstar = GOLD["lj_rstar"]
+    s = H.two_atoms(rstar)
+    o = oracle.OracleSystem(s)
+    sv = np.zeros((2, 3))
+    sv[1] = [1.0, 0.0, 0.0]
+    res = oracle.bead(o, s.R1, geom=0, brute=True, s=sv)
+    assert res["U"][0] == pytest.approx(GOLD["lj_u_at_rstar"], rel=1e-6)
+    assert np.abs(res["F"]).max() < 2e-4          # zero force at the minimum (c6/c12 are float32)
+    # along-axis curvature u''(r*) = 72 eps/(2^(1/3) sigma^2); transverse u'/r = 0
+    assert res["Hs"][1, 0] == pytest.approx(GOLD["lj_upp_at_rstar"], rel=1e-5)
+    assert res["Hs"][0, 0] == pytest.approx(-GOLD["lj_upp_at_rstar"], rel=1e-5)
+    sv[1] = [0.0, 1.0, 0.0]
+    res = oracle.bead(o, s.R1, geom=0, brute=True, s=sv)
+    assert np.abs(res["Hs"]).max() < 2e-3
+
+
+def test_P1_lj_potential_shift(oracle):
+    """lj_shift=1 makes U_LJ(r_c) = 0 and leaves the force unchanged."""
+    r = 0.9999999
+    a = oracle.bead(oracle.OracleSystem(H.two_atoms(r, lj_shift=1)), H.two_atoms(r).R1, geom=0, brute=True)
+    b = oracle.bead(oracle.OracleSystem(H.two_atoms(r, lj_shift=0)), H.two_atoms(r).R1, geom=0, brute=True)
+    assert abs(a["U"][0]) < 1e-8
+    assert abs(b["U"][0]) > 1e-3
+    assert np.allclose(a["F"], b["F"], rtol=0, atol=1e-14)
+    # beyond the cutoff: no pair
+    c = oracle.bead(oracle.OracleSystem(H.two_atoms(1.0000001)), H.two_atoms(1.0000001).R1, geom=0, brute=True)
+    assert c["npairs"] == 0 and np.abs(c["F"]).max() == 0.0
+
+
+@pytest.mark.parametrize("r", [0.25, 0.50, 0.90])
+def test_P2_reaction_field_closed_form(oracle, r):
+    s = H.two_atoms(r, eps=0.0, q=(-0.82, 0.41))
+    o = oracle.OracleSystem(s)
+    res = oracle.bead(o, s.R1, geom=0, brute=True)
+    qs = float(np.float32(-0.82)) * float(np.float32(0.41)) / (-0.82 * 0.41)   # float32 charges
+    assert res["U"][1] == pytest.approx(GOLD["rf_u_r=%.2f" % r] * qs, rel=1e-9)
+    assert res["F"][1, 0] == pytest.approx(GOLD["rf_F_r=%.2f" % r] * qs, rel=1e-9)
+    assert res["U"][0] == 0.0
+
+
+def test_P2_reaction_field_at_cutoff(oracle):
+    r = 1.0 - 1e-10
+    s = H.two_atoms(r, eps=0.0, q=(-0.82, 0.41))
+    res = oracle.bead(oracle.OracleSystem(s), s.R1, geom=0, brute=True)
+    qs = float(np.float32(-0.82)) * float(np.float32(0.41)) / (-0.82 * 0.41)
+    assert abs(res["U"][1]) < 1e-7                                   # u(r_c) = 0
+    assert res["F"][1, 0] == pytest.approx(GOLD["rf_F_at_rc"] * qs, rel=1e-7)
+    # eps_rf <= 0 means infinity: k_rf = 1/(2 rc^3), force vanishes at r_c
+    s2 = H.two_atoms(r, eps=0.0, q=(-0.82, 0.41), eps_rf=0.0)
+    res2 = oracle.bead(oracle.OracleSystem(s2), s2.R1, geom=0, brute=True)
+    assert abs(res2["F"][1, 0]) < 1e-6 and abs(res2["U"][1]) < 1e-7
+
+
+# ---------------------------------------------------------------- P3 HVP vs finite differences
+def _clear_of_cutoff(make, tol=2e-4):
+    """G9: FD pins need configurations with no pair at the cutoff; take the first seed that has none."""
+    for seed in range(1, 50):
+        s = make(seed)
+        if H.pairs_near_cutoff(s, s.R1, tol) == 0:
+            return s
+    raise RuntimeError("no seed without a pair at the cutoff")
+
+
+def _systems():
+    return [_clear_of_cutoff(lambda sd: H.lj_cluster(32, seed=sd)),
+            _clear_of_cutoff(lambda sd: H.tiny_water(seed=sd)),
+            _clear_of_cutoff(lambda sd: H.tiny_chain(seed=sd)),
+            _clear_of_cutoff(lambda sd: H.lj_cluster(27, seed=sd, masses=np.linspace(5, 40, 27)))]
+
+
+@pytest.mark.parametrize("idx", range(3))
+def test_P3_hvp_vs_central_difference_of_forces(oracle, idx):
+    s = _systems()[idx]
+    assert H.pairs_near_cutoff(s, s.R1, 2e-4) == 0, "G9: move the seed, a pair sits at the cutoff"
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(5)
+    sv = rng.normal(0, 1, (s.n_atoms, 3))
+    res = oracle.bead(o, s.R1, geom=0, brute=True, s=sv)
+    eps = 1e-6
+    Fp = oracle.bead(o, s.R1 + eps * sv, geom=0, brute=True)["F"]
+    Fm = oracle.bead(o, s.R1 - eps * sv, geom=0, brute=True)["F"]
+    Hs_fd = -(Fp - Fm) / (2 * eps)
+    assert H.rms_rel(res["Hs"], Hs_fd) < 2e-7
+    # each term type separately has to be there: zero direction on all but one atom
+    sv1 = np.zeros_like(sv)
+    sv1[3] = [0.3, -0.2, 0.9]
+    r1 = oracle.bead(o, s.R1, geom=0, brute=True, s=sv1)["Hs"]
+    Fp = oracle.bead(o, s.R1 + eps * sv1, geom=0, brute=True)["F"]
+    Fm = oracle.bead(o, s.R1 - eps * sv1, geom=0, brute=True)["F"]
+    assert H.rms_rel(r1, -(Fp - Fm) / (2 * eps)) < 2e-7
+
+
+def test_P3_force_is_minus_gradient_of_energy(oracle):
+    """F = -dU/dR by central differences of the oracle's own energy."""
+    for s in _systems()[:3]:
+        o = oracle.OracleSystem(s)
+        F = oracle.bead(o, s.R1, geom=0, brute=True)["F"]
+        rng = np.random.default_rng(11)
+        for _ in range(6):
+            i, a = int(rng.integers(s.n_atoms)), int(rng.integers(3))
+            e = 1e-6
+            Xp, Xm = s.R1.copy(), s.R1.copy()
+            Xp[i, a] += e
+            Xm[i, a] -= e
+            up = oracle.bead(o, Xp, geom=0, brute=True)["U"].sum()
+            um = oracle.bead(o, Xm, geom=0, brute=True)["U"].sum()
+            assert F[i, a] == pytest.approx(-(up - um) / (2 * e), rel=2e-6, abs=2e-5)
+
+
+# ---------------------------------------------------------------- P4 / P5 gradient of V_eff
+def _tiny_path(oracle, s, N, seed=0, noise=True):
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, N, lambda X: oracle.bead(o, X, geom=0, brute=True)["F"], seed=seed, noise=noise,
+                        dtype=np.float64)
+    return o, R
+
+
+@pytest.mark.parametrize("idx", [2, 3])
+def test_P4_gradient_vs_finite_difference_of_veff(oracle, idx):
+    s = _systems()[idx]
+    o, R = _tiny_path(oracle, s, 5)
+    v, G = oracle.veff_grad(o, R, geom=0, brute=True)
+    rng = np.random.default_rng(3)
+    e = 2e-7
+    worst = 0.0
+    for _ in range(40):
+        n, i, a = int(rng.integers(R.shape[0])), int(rng.integers(s.n_atoms)), int(rng.integers(3))
+        Rp, Rm = R.copy(), R.copy()
+        Rp[n, i, a] += e
+        Rm[n, i, a] -= e
+        fd = (oracle.veff_grad(o, Rp, geom=0, brute=True)[0] - oracle.veff_grad(o, Rm, geom=0, brute=True)[0]) / (2 * e)
+        worst = max(worst, abs(fd - G[n, i, a]) / max(abs(G[n, i, a]), 1.0))
+    assert worst < 5e-6
+
+
+def test_P5_paper_equations_5_6_7(oracle):
+    """-grad equals eqs (5),(6),(7) of the paper with the bracket evaluated by central differences."""
+    s = _systems()[3]                     # unequal masses
+    o, R = _tiny_path(oracle, s, 5)
+    v, G, parts = oracle.veff_grad(o, R, geom=0, brute=True, want_parts=True)
+    N = R.shape[0]
+    m = s.mass.astype(float)[:, None]
+    K = m * s.nu / (2 * s.dt_path)
+    a = s.dt_path / (m * s.nu)
+    force = lambda X: oracle.bead(o, X, geom=0, brute=True)["F"]
+    F = [force(R[n]) for n in range(N)]
+    eps = 1e-4
+
+    def bracket(n):
+        eta = R[n + 1] - R[n] - a * F[n]
+        sc = eps / np.abs(eta).max()
+        return (force(R[n] + sc * eta) - force(R[n] - sc * eta)) / (4 * sc)
+
+    Feff = np.zeros_like(R)
+    Feff[0] = 0.5 * F[0] + K * (R[1] - R[0]) + bracket(0)                                   # eq. (6)
+    for n in range(1, N - 1):
+        Feff[n] = -K * (2 * R[n] - R[n - 1] - R[n + 1]) + 0.5 * (F[n - 1] - F[n]) + bracket(n)  # eq. (5)
+    Feff[N - 1] = -K * (R[N - 1] - R[N - 2]) + 0.5 * F[N - 2]                               # eq. (7)
+    assert H.rms_rel(-G, Feff) < 1e-6
+    for n in range(N):
+        assert H.rms_rel(-G[n], Feff[n]) < 5e-6
+
+
+# ---------------------------------------------------------------- P6 / P7 invariants
+@pytest.mark.parametrize("idx", range(3))
+def test_P6_newton_third_law_and_translation(oracle, idx):
+    s = _systems()[idx]
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(9)
+    sv = rng.normal(0, 1, (s.n_atoms, 3))
+    res = oracle.bead(o, s.R1, geom=0, brute=True, s=sv)
+    scale = np.abs(res["F"]).max()
+    assert np.abs(res["F"].sum(0)).max() < 1e-11 * scale
+    assert np.abs(res["Hs"].sum(0)).max() < 1e-10 * np.abs(res["Hs"]).max()
+    t = np.tile([[0.3, -1.0, 0.7]], (s.n_atoms, 1))
+    Ht = oracle.bead(o, s.R1, geom=0, brute=True, s=t)["Hs"]
+    assert np.abs(Ht).max() < 1e-9 * np.abs(res["Hs"]).max()
+
+
+@pytest.mark.parametrize("idx", range(3))
+def test_P7_hessian_symmetry(oracle, idx):
+    s = _systems()[idx]
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(10)
+    a = rng.normal(0, 1, (s.n_atoms, 3))
+    b = rng.normal(0, 1, (s.n_atoms, 3))
+    Ha = oracle.bead(o, s.R1, geom=0, brute=True, s=a)["Hs"]
+    Hb = oracle.bead(o, s.R1, geom=0, brute=True, s=b)["Hs"]
+    assert (b * Ha).sum() == pytest.approx((a * Hb).sum(), rel=1e-10)
+
+
+# ---------------------------------------------------------------- P8 / P9 / P10 the path
+def test_P8_equipartition_on_generated_path(oracle):
+    """On a Brownian path E_spring/(3Q(N-1)) = kT/2 (pins K, L^n scale and reading G1)."""
+    s = W.config1()
+    o = oracle.OracleSystem(s)
+    N = 6
+    R = W.brownian_path(s, N, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0, dtype=np.float64)
+    v, G, parts = oracle.veff_grad(o, R, geom=0, want_parts=True)
+    dof = 3 * s.n_atoms * (N - 1)
+    ratio = parts["E_spring"] / dof / (0.5 * W.KB * s.temperature)
+    assert abs(ratio - 1.0) < 4.0 * np.sqrt(2.0 / dof)
+    assert v == pytest.approx(parts["U1"] + parts["E_spring"], rel=1e-14)
+
+
+def test_P9_noise_free_euler_path(oracle):
+    s = H.tiny_chain()
+    o, R = _tiny_path(oracle, s, 5, noise=False)
+    v, G, parts = oracle.veff_grad(o, R, geom=0, brute=True, want_parts=True)
+    F1 = oracle.bead(o, R[0], geom=0, brute=True)
+    assert parts["E_spring"] < 1e-18
+    assert np.abs(parts["eta"]).max() < 1e-15
+    assert v == pytest.approx(F1["U"].sum(), rel=1e-13)
+    assert H.rms_rel(G[0], -F1["F"]) < 1e-9
+    assert np.abs(G[1:]).max() < 1e-8 * np.abs(G[0]).max()
+
+
+def test_P10_special_cases_N1_N2(oracle):
+    s = H.tiny_chain()
+    o, R = _tiny_path(oracle, s, 2)
+    b = oracle.bead(o, R[0], geom=0, brute=True)
+    v1, G1 = oracle.veff_grad(o, R[:1], geom=0, brute=True)
+    assert v1 == pytest.approx(b["U"].sum(), rel=1e-14)
+    assert np.allclose(G1[0], -b["F"], rtol=0, atol=1e-12 * np.abs(b["F"]).max())
+    v2, G2, p2 = oracle.veff_grad(o, R, geom=0, brute=True, want_parts=True)
+    m = s.mass.astype(float)[:, None]
+    K = m * s.nu / (2 * s.dt_path)
+    eta = R[1] - R[0] - s.dt_path / (m * s.nu) * b["F"]
+    assert np.allclose(G2[1], K * eta, rtol=1e-12, atol=1e-9)
+    assert v2 == pytest.approx(b["U"].sum() + (0.5 * K * eta ** 2).sum(), rel=1e-13)
+
+
+def test_P11_zero_length_harmonic_dimer(oracle):
+    """b0 = 0: U = k|r1-r2|^2/2, H = k[[I,-I],[-I,I]] constant; V_eff is a homogeneous quadratic form in
+    the bead coordinates, hence x . grad V_eff = 2 V_eff (Euler) and grad is linear in x."""
+    k = 1234.5
+    X = np.array([[1.0, 1.0, 1.0], [1.13, 0.95, 1.08]])
+    s = H.make_system("dimer", [5.0] * 3, X, [12.0, 3.0], [0, 0], [0, 0], [0.3], [0.0], bonds=[[0, 1]],
+                      bpar=[[0.0, k]], r_cut=1.0)
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(4)
+    sv = rng.normal(0, 1, (2, 3))
+    res = oracle.bead(o, X, geom=0, brute=True, s=sv)
+    assert np.allclose(res["Hs"][0], k * (sv[0] - sv[1]), rtol=1e-12)
+    assert np.allclose(res["Hs"][1], -k * (sv[0] - sv[1]), rtol=1e-12)
+    assert res["U"][2] == pytest.approx(0.5 * k * ((X[0] - X[1]) ** 2).sum(), rel=1e-13)
+    N = 4
+    R = rng.normal(0, 0.05, (N, 2, 3)) + 1.0
+    c = np.array([1.0, 1.0, 1.0])          # V_eff depends on r1-r2 and bead differences only
+    v, G = oracle.veff_grad(o, R, geom=0, brute=True)
+    assert ((R - c) * G).sum() == pytest.approx(2.0 * v, rel=1e-11)
+    v3, G3 = oracle.veff_grad(o, c + 3.0 * (R - c), geom=0, brute=True)
+    assert v3 == pytest.approx(9.0 * v, rel=1e-11)
+    assert np.allclose(G3, 3.0 * G, rtol=1e-10, atol=1e-9)
+
+
+# ---------------------------------------------------------------- P12 integrator
+def test_P12_velocity_verlet_invariants(oracle):
+    s = H.lj_cluster(32)
+    o, R = _tiny_path(oracle, s, 4)
+    rng = np.random.default_rng(8)
+    V = rng.normal(0, 1, R.shape) * np.sqrt(W.KB * 120.0 / s.mass.astype(float))[None, :, None]
+    dt = 0.001
+    R1, V1, e1 = oracle.step(o, R, V, dt, 200, geom=0, brute=True)
+    R2, V2, e2 = oracle.step(o, R, V, dt / 2, 400, geom=0, brute=True)
+    fl1 = np.std(e1[:, 2])
+    fl2 = np.std(e2[::2, 2])
+    assert fl1 < 2e-2 * np.std(e1[:, 1])                  # total energy conserved vs kinetic swings
+    assert 2.5 < fl1 / fl2 < 6.0                          # fluctuation ~ dt^2
+    assert abs(e1[-1, 2] - e1[0, 2]) < 5 * fl1 + 1e-9     # no drift
+    # time reversal
+    Rb, Vb, _ = oracle.step(o, R1, -V1, dt, 200, geom=0, brute=True)
+    assert np.abs(Rb - R).max() < 1e-9
+    assert np.abs(Vb + V).max() < 1e-6
+
+
+# ---------------------------------------------------------------- P13 + G8 neighbour sets
+@pytest.mark.parametrize("mk", ["c1", "c2", "tiny", "edge"])
+def test_P13_cell_list_equals_brute_force(oracle, mk):
+    if mk == "c1":
+        s = W.config1()
+    elif mk == "c2":
+        s = W.config2()
+    elif mk == "tiny":
+        s = H.tiny_chain()
+    else:
+        s = H.lj_cluster(64, L=2.0001, r_cut=1.0)       # box barely above 2 r_c
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(1)
+    X = s.R1 + rng.integers(-2, 3, (s.n_atoms, 1)) * np.asarray(s.box, float)   # unwrapped images
+    for geom in (0, 1):
+        pb = oracle.pairs(o, X, geom=geom, brute=True)
+        pc = oracle.pairs(o, X, geom=geom, brute=False)
+        assert pb.shape == pc.shape and (pb == pc).all()
+    # FP32-contract set differs from the FP64 set only by pairs at the cutoff / the float rounding of X
+    p0 = oracle.pairs(o, s.R1.astype(np.float32).astype(np.float64), geom=0)
+    p1 = oracle.pairs(o, s.R1, geom=1)
+    a = set(map(tuple, p0.tolist()))
+    b = set(map(tuple, p1.tolist()))
+    assert len(a ^ b) <= max(2, len(a) // 100000)
+    # no excluded pair is ever listed
+    ex = {(i, int(j)) for i in range(s.n_atoms) for j in s.excl_list[s.excl_start[i]:s.excl_start[i + 1]]}
+    assert not (b & ex)
+
+
+def test_G8_wrap_cells_and_stable_sort(oracle):
+    s = W.config2()
+    rng = np.random.default_rng(2)
+    X = (s.R1 + rng.integers(-3, 4, (s.n_atoms, 3)) * np.asarray(s.box, float)).astype(np.float32)
+    xw = oracle.wrap(X, s.box)
+    L = s.box.astype(np.float32)
+    assert (xw >= 0).all() and (xw < L).all()
+    d = (xw.astype(float) - X.astype(float)) / L
+    assert np.abs(d - np.round(d)).max() < 1e-6           # same point modulo the box
+    dims = oracle.grid_dims(s.n_atoms, s.box, 8, 0.1)
+    assert dims[0] >= 1 and dims[2] == int(np.floor(float(L[2]) / np.float32(0.1)))
+    cell = oracle.cell_ids(xw, s.box, dims)
+    assert cell.min() >= 0 and cell.max() < dims[0] * dims[1] * dims[2]
+    cz = cell % dims[2]
+    assert np.abs((cz + 0.5) * (L[2] / dims[2]) - xw[:, 2]).max() <= 0.5 * L[2] / dims[2] * 1.001
+    perm = oracle.stable_sort_by_cell(cell, dims[0] * dims[1] * dims[2])
+    assert sorted(perm.tolist()) == list(range(s.n_atoms))
+    key = cell[perm].astype(np.int64) * s.n_atoms + perm
+    assert (np.diff(key) > 0).all()                        # sorted by cell, ties by ascending index
+
+
+def test_geom1_matches_geom0_physics(oracle):
+    """The FP32-contract mode does its physics in FP64: same V_eff/grad as pure FP64 on float inputs."""
+    s = H.tiny_chain()
+    o, R = _tiny_path(oracle, s, 4)
+    R32 = R.astype(np.float32).astype(np.float64)
+    assert H.pairs_near_cutoff(s, R32[0], 1e-5) == 0
+    v0, G0 = oracle.veff_grad(o, R32, geom=0, brute=True)
+    v1, G1 = oracle.veff_grad(o, R32, geom=1, brute=False)
+    assert v1 == pytest.approx(v0, rel=1e-12)
+    assert H.rms_rel(G1, G0) < 1e-10

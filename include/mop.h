@@ -1,0 +1,150 @@
+/*
+ * mop.h -- C-ABI of libmop_b200: the data-parallel hot path of the
+ * metadynamics-of-paths (MoP) method, arxiv 2501.11962, for one NVIDIA B200.
+ *
+ * What the library computes (citations are lines of the paper text PAPER.md):
+ *   - the Onsager-Machlup effective potential of an N-bead discretised path,
+ *       V_eff = U(R^1) + sum_{n=1}^{N-1} sum_i K_i/2 |R^{n+1}_i - R^n_i - L^n_i|^2     eq. (3)
+ *     with K_i = m_i nu / (2 dt) and L^n_i = dt/(m_i nu) F^n_i
+ *     (the printed L^n is inverted; reading G1 in DESIGN.md: eqs (5)-(7) need K L/F = 1/2),
+ *     F^n = -grad U(R^n);
+ *   - its gradient dV_eff/dR^n = -F_eff^n, F_eff^n as in eqs (5),(6),(7), with the
+ *     finite-difference bracket [F(R+eps eta)-F(R-eps eta)]/(4 eps) replaced by its eps->0 limit
+ *     -(1/2) H(R^n) eta^n, computed analytically (eta^n = R^{n+1}-R^n-L^n);
+ *   - velocity-Verlet path MD of the polymer, M d2R^n/dt2 = F_eff^n, eq. (4).
+ * U is BASELINE.json's force field: Lennard-Jones 12-6 (optional potential shift) + reaction-field
+ * Coulomb with a plain cutoff r_cut, harmonic bonds and harmonic angles, explicit exclusions.
+ *
+ * Units: nm, ps, u, kJ/mol, e (1 kJ/mol = 1 u nm^2/ps^2).  Coulomb constant 138.935458 kJ mol^-1 nm e^-2.
+ *
+ * Conventions
+ *   - "HOST" / "DEVICE" says where a pointer must live.  Device pointers are plain CUDA device
+ *     addresses on `params.device`; the caller (e.g. torch) owns R, V, grad; the library owns
+ *     everything else and frees it in mop_destroy.
+ *   - All work is enqueued on `params.stream`; a call synchronises the stream only where stated.
+ *   - No exceptions or abort() cross the ABI: every call returns a mop_status; CUDA errors are
+ *     sticky per context; mop_last_error gives a text.
+ *   - Calls on one context are not thread-safe.
+ *   - There is no CPU fallback: without a CUDA device mop_create returns MOP_ERR_CUDA.
+ */
+#ifndef MOP_B200_H
+#define MOP_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mop_ctx mop_ctx; /* opaque; one per (device, system) */
+
+typedef enum {
+    MOP_OK = 0,
+    MOP_ERR_INVALID_ARG = 1,   /* bad size, pointer, index, non-positive mass, asymmetric exclusions */
+    MOP_ERR_NO_TOPOLOGY = 2,   /* eval/step before mop_set_topology */
+    MOP_ERR_BOX_TOO_SMALL = 3, /* min(box) < 2 (r_cut + r_buf): the in-range periodic image would not be unique */
+    MOP_ERR_OOM = 4,           /* device allocation failed or a pair-list buffer overflowed */
+    MOP_ERR_CUDA = 5,          /* any CUDA runtime error (sticky), or no device */
+    MOP_ERR_NONFINITE = 6      /* V_eff came out NaN/Inf (overlapping atoms) */
+} mop_status;
+
+/* Problem statement of PAPER.md:36-52: Q atoms, N beads at path spacing dt, friction nu.  Copied at create. */
+typedef struct {
+    int n_atoms;      /* Q >= 1 */
+    int n_beads;      /* N >= 1 */
+    float box[3];     /* rectangular periodic box (nm) */
+    float r_cut;      /* nonbonded cutoff (nm), > 0 */
+    float r_buf;      /* Verlet buffer (nm), >= 0.  0: the pair list is rebuilt in every evaluation.  > 0: the
+                         list (built with r_cut + r_buf) is reused until an atom has moved more than r_buf/2 */
+    float eps_rf;     /* reaction-field dielectric; <= 0 means infinity (k_rf = 1/(2 r_cut^3)) */
+    int lj_shift;     /* 1: potential-shift the LJ energy so that U_LJ(r_cut) = 0 (forces unchanged) */
+    double dt_path;   /* path spacing Delta t (ps): enters K_i and L^n only */
+    double nu;        /* Smoluchowski friction nu (1/ps): enters K_i and L^n only */
+    int device;       /* CUDA ordinal */
+    void *stream;     /* cudaStream_t all work is enqueued on (NULL: the legacy default stream) */
+} mop_params;
+
+/* HOST pointers; copied to the device inside mop_set_topology; the caller keeps ownership. */
+typedef struct {
+    const float *mass;   /* [Q] u, > 0 (physical = fictitious masses, reading G4) */
+    const float *charge; /* [Q] e */
+    const int *type;     /* [Q] in [0, n_types) */
+    int n_types;         /* 1..64 */
+    const float *c6;     /* [n_types*n_types] symmetric, kJ/mol nm^6 */
+    const float *c12;    /* [n_types*n_types] symmetric, kJ/mol nm^12 */
+    int n_bonds;
+    const int *bond_ij;        /* [n_bonds][2] atom indices */
+    const float *bond_b0_kb;   /* [n_bonds][2] = (b0 nm, k_b kJ/mol/nm^2); u = k_b/2 (r-b0)^2 */
+    int n_angles;
+    const int *angle_ijk;      /* [n_angles][3], j central */
+    const float *angle_t0_kt;  /* [n_angles][2] = (theta0 rad, k_theta kJ/mol/rad^2); u = k_t/2 (theta-theta0)^2 */
+    const int *excl_start;     /* CSR [Q+1] (may be NULL when there are no exclusions) */
+    const int *excl_list;      /* symmetric, sorted; an excluded pair gets NO nonbonded term (no RF correction, G10) */
+} mop_topology;
+
+/* Creates a context for (device, Q, N, box, cutoffs); allocates nothing that depends on the topology.
+ * Errors: INVALID_ARG, BOX_TOO_SMALL, CUDA, OOM. */
+mop_status mop_create(mop_ctx **out, const mop_params *p);
+
+/* Validates and uploads the topology; may be called again to replace it.  Synchronises the stream. */
+mop_status mop_set_topology(mop_ctx *c, const mop_topology *t);
+
+/* V_eff (eq. 3) and its gradient (= -F_eff of eqs 5,6,7) for the whole path.
+ *   R_dev    DEVICE [N][Q][3] float; beads image-consistent (an atom's coordinate is continuous along the
+ *            path; the library wraps only its internal sorted copy).  Read only.
+ *   veff_out HOST; non-NULL: the call synchronises the stream and stores V_eff (kJ/mol);
+ *            NULL: fully asynchronous, the value stays in the context (mop_get_stats).
+ *   grad_dev DEVICE [N][Q][3] float, dV_eff/dR^n_i in kJ/mol/nm, caller-allocated; NULL: not written.
+ * Passes: S0 bin+sort, S1 pair list, S2 nonbonded force, S3 bonded force,
+ * S4 eta + spring energy, S5 nonbonded H.eta, S6 bonded H.eta, S7 assembly.
+ * Errors: NO_TOPOLOGY, INVALID_ARG, OOM (list overflow, reported at a synchronising call), CUDA, NONFINITE. */
+mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double *veff_out, float *grad_dev);
+
+/* n_steps velocity-Verlet steps of eq. (4) with F_eff = -grad V_eff and masses m_i, step dt_pmd (ps):
+ *   v += dt/2 F_eff/m ; R += dt v ; F_eff(R) ; v += dt/2 F_eff/m.
+ * R_dev, V_dev DEVICE [N][Q][3] float, updated in place.  The gradient at the incoming R is evaluated at the
+ * start of every call (n_steps + 1 evaluations per call).  Asynchronous. */
+mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps);
+
+/* NULL-safe; frees all library-owned memory. */
+void mop_destroy(mop_ctx *c);
+
+/* Static or context-owned text for the last non-OK status (c may be NULL: creation errors). */
+const char *mop_last_error(const mop_ctx *c);
+
+/* ---- optional, for tests and benches ------------------------------------------------------------- */
+
+/* Synchronises.  out[0]=V_eff, [1]=U(R^1), [2]=E_spring, [3]=U_lj(R^1), [4]=U_coul(R^1), [5]=U_bond(R^1),
+ * [6]=U_angle(R^1), [7]=kinetic energy after the last mop_step, [8]=pair-list rebuilds so far,
+ * [9]=cluster-pair entries in the current list, [10]=list units, [11]=exclusion masks,
+ * [12]=pair slots evaluated per nonbonded pass (entries * 8 * 32), [13]=kernel launches so far,
+ * [14],[15] reserved. */
+mop_status mop_get_stats(mop_ctx *c, double out[16]);
+
+/* Copies an internal array of the last evaluation to HOST memory (synchronises).  `what`:
+ *   "dims"  int[8]: nx, ny, nz (search grid), slots per bead S (padded, multiple of 32), force beads nf,
+ *           cluster size 32, i-cluster size 8, 0
+ *   "cell"  int[nf][Q]   cell id of every atom, cell = (cx*ny+cy)*nz+cz (reading G8)
+ *   "perm"  int[nf][S]   original atom index held by each sorted slot, -1 for padding (stable sort, G13)
+ *   "xq"    float[nf][S][4] wrapped coordinates + charge in sorted order
+ *   "F"     float[nf][Q][3] physical force F^n in ORIGINAL atom order
+ *   "eta"   float[nf][Q][3] eta^n in original order;  "Heta" float[nf][Q][3] H^n eta^n likewise
+ * bytes must equal the size of the array.  Errors: INVALID_ARG. */
+mop_status mop_debug_get(mop_ctx *c, const char *what, void *host_buf, size_t bytes);
+
+/* In-range (r2 < r_cut^2 under the FP32 predicate G8), non-excluded atom pairs of bead `bead` of the last
+ * evaluation, found by walking the pair list with the force kernel's own predicate.  Writes up to `cap` pairs
+ * (original indices, unordered) to HOST pairs[2*k], pairs[2*k+1] (may be NULL with cap 0) and the total count
+ * to *n_pairs.  Synchronises. */
+mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long long cap, long long *n_pairs);
+
+/* Physical force and H.s of ONE configuration treated as bead 1 of a context with n_beads == 1 is what
+ * mop_eval_veff_grad already gives (grad = -F).  For a user-supplied direction s:
+ *   R_dev, s_dev DEVICE [Q][3]; F_dev, Hs_dev DEVICE [Q][3] outputs (either may be NULL).  Uses bead slot 0.
+ * This is the pass-2 kernel with eta := s.  Asynchronous. */
+mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float *s_dev, float *F_dev, float *Hs_dev);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOP_B200_H */

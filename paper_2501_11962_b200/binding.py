@@ -1,0 +1,229 @@
+"""Thin ctypes binding of libmop_b200.so (include/mop.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C-ABI; torch is used for device
+memory and the stream handle.  There is no CPU fallback: if the library is missing or cannot be
+loaded this module raises, and a context cannot be created without a CUDA device.
+Names follow the C-ABI: mop_create / mop_set_topology / mop_eval_veff_grad / mop_step / mop_destroy.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MOP_OK = 0
+STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "MOP_ERR_BOX_TOO_SMALL",
+          4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
+EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
+           "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp"]
+
+
+class MopError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("%s: %s" % (STATUS.get(status, status), msg))
+        self.status = status
+
+
+class mop_params(C.Structure):
+    _fields_ = [("n_atoms", C.c_int), ("n_beads", C.c_int), ("box", C.c_float * 3), ("r_cut", C.c_float),
+                ("r_buf", C.c_float), ("eps_rf", C.c_float), ("lj_shift", C.c_int), ("dt_path", C.c_double),
+                ("nu", C.c_double), ("device", C.c_int), ("stream", C.c_void_p)]
+
+
+class mop_topology(C.Structure):
+    _fields_ = [("mass", C.c_void_p), ("charge", C.c_void_p), ("type", C.c_void_p), ("n_types", C.c_int),
+                ("c6", C.c_void_p), ("c12", C.c_void_p), ("n_bonds", C.c_int), ("bond_ij", C.c_void_p),
+                ("bond_b0_kb", C.c_void_p), ("n_angles", C.c_int), ("angle_ijk", C.c_void_p),
+                ("angle_t0_kt", C.c_void_p), ("excl_start", C.c_void_p), ("excl_list", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib_path():
+    return _build.LIB
+
+
+def load(build_if_missing=True):
+    """Loads the C-ABI library (building it with nvcc when it is missing or stale).  Raises if unavailable."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        _build.build()
+    if not os.path.exists(_build.LIB):
+        raise RuntimeError("libmop_b200.so is not built (run python -m paper_2501_11962_b200.build); "
+                           "there is no CPU fallback")
+    L = C.CDLL(_build.LIB)
+    L.mop_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(mop_params)]
+    L.mop_set_topology.argtypes = [C.c_void_p, C.POINTER(mop_topology)]
+    L.mop_eval_veff_grad.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+    L.mop_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int]
+    L.mop_destroy.argtypes = [C.c_void_p]
+    L.mop_destroy.restype = None
+    L.mop_last_error.argtypes = [C.c_void_p]
+    L.mop_last_error.restype = C.c_char_p
+    L.mop_get_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+    L.mop_debug_get.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p, C.c_size_t]
+    L.mop_debug_pairs.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_longlong, C.POINTER(C.c_longlong)]
+    L.mop_force_hvp.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
+              "mop_debug_pairs", "mop_force_hvp"):
+        getattr(L, n).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _np(a, dtype, shape=None):
+    a = np.ascontiguousarray(np.asarray(a, dtype=dtype))
+    return a if shape is None else a.reshape(shape)
+
+
+class Mop:
+    """One context (device, system).  `system` carries the attributes of workloads.System."""
+
+    def __init__(self, system, n_beads, device=0, r_buf=0.0, stream=None):
+        import torch
+        self.torch = torch
+        self.L = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the MoP hot path has no CPU fallback")
+        self.device = torch.device("cuda", device)
+        self.Q, self.N = int(system.n_atoms), int(n_beads)
+        self.nf = max(self.N - 1, 1)
+        p = mop_params()
+        p.n_atoms, p.n_beads = self.Q, self.N
+        for d in range(3):
+            p.box[d] = float(np.float32(system.box[d]))
+        p.r_cut, p.r_buf = float(system.r_cut), float(r_buf)
+        p.eps_rf, p.lj_shift = float(system.eps_rf), int(system.lj_shift)
+        p.dt_path, p.nu = float(system.dt_path), float(system.nu)
+        p.device = device
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.stream = st
+        p.stream = C.c_void_p(st.cuda_stream)
+        self.ctx = C.c_void_p()
+        s = self.L.mop_create(C.byref(self.ctx), C.byref(p))
+        if s != MOP_OK:
+            raise MopError(s, (self.L.mop_last_error(None) or b"").decode())
+        self.set_topology(system)
+
+    def _check(self, s):
+        if s != MOP_OK:
+            raise MopError(s, (self.L.mop_last_error(self.ctx) or b"").decode())
+
+    def mop_set_topology(self, system):
+        t = mop_topology()
+        keep = []
+
+        def arr(x, dtype, shape=None):
+            a = _np(x, dtype, shape)
+            keep.append(a)
+            return a.ctypes.data_as(C.c_void_p) if a.size else None
+
+        t.mass, t.charge, t.type = arr(system.mass, np.float32), arr(system.charge, np.float32), arr(system.type, np.int32)
+        t.n_types = int(system.n_types)
+        t.c6, t.c12 = arr(system.c6, np.float32), arr(system.c12, np.float32)
+        b = _np(system.bond_ij, np.int32, (-1, 2))
+        t.n_bonds = b.shape[0]
+        t.bond_ij, t.bond_b0_kb = arr(b, np.int32), arr(system.bond_b0_kb, np.float32)
+        a = _np(system.angle_ijk, np.int32, (-1, 3))
+        t.n_angles = a.shape[0]
+        t.angle_ijk, t.angle_t0_kt = arr(a, np.int32), arr(system.angle_t0_kt, np.float32)
+        es = _np(system.excl_start, np.int32)
+        keep.append(es)
+        t.excl_start = es.ctypes.data_as(C.c_void_p)
+        t.excl_list = arr(system.excl_list, np.int32)
+        self._check(self.L.mop_set_topology(self.ctx, C.byref(t)))
+
+    set_topology = mop_set_topology
+
+    def _dev(self, R, shape):
+        torch = self.torch
+        if not isinstance(R, torch.Tensor):
+            R = torch.as_tensor(np.ascontiguousarray(R, dtype=np.float32))
+        R = R.to(device=self.device, dtype=torch.float32).contiguous()
+        assert tuple(R.shape) == tuple(shape), (R.shape, shape)
+        return R
+
+    def mop_eval_veff_grad(self, R, want_grad=True, sync=True, grad_out=None):
+        """R: [N][Q][3] float32 (torch cuda tensor, or anything castable).  Returns (veff | None, grad | None)."""
+        R = self._dev(R, (self.N, self.Q, 3))
+        grad = grad_out
+        if want_grad and grad is None:
+            grad = self.torch.empty_like(R)
+        v = C.c_double(0.0)
+        self._check(self.L.mop_eval_veff_grad(self.ctx, _ptr(R), C.byref(v) if sync else None,
+                                              _ptr(grad) if want_grad else None))
+        return (v.value if sync else None), (grad if want_grad else None)
+
+    def mop_step(self, R, V, dt_pmd, n_steps):
+        """In-place velocity Verlet on torch cuda tensors R, V [N][Q][3] float32."""
+        assert R.is_cuda and V.is_cuda and R.is_contiguous() and V.is_contiguous()
+        assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
+        self._check(self.L.mop_step(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps)))
+
+    def mop_force_hvp(self, R1, s=None):
+        """Physical force (and H.s for a direction s) of one configuration [Q][3].  Returns (F, Hs) tensors."""
+        R1 = self._dev(R1, (self.Q, 3))
+        F = self.torch.empty_like(R1)
+        Hs = None
+        sd = None
+        if s is not None:
+            sd = self._dev(s, (self.Q, 3))
+            Hs = self.torch.empty_like(R1)
+        self._check(self.L.mop_force_hvp(self.ctx, _ptr(R1), _ptr(sd), _ptr(F), _ptr(Hs)))
+        return F, Hs
+
+    def mop_get_stats(self):
+        out = (C.c_double * 16)()
+        self._check(self.L.mop_get_stats(self.ctx, out))
+        k = ["veff", "U1", "E_spring", "U_lj", "U_coul", "U_bond", "U_angle", "E_kin", "rebuilds", "entries", "units",
+             "masks", "pair_slots", "launches"]
+        return dict(zip(k, list(out)[:14]))
+
+    def dims(self):
+        d = np.zeros(8, np.int32)
+        self._check(self.L.mop_debug_get(self.ctx, b"dims", d.ctypes.data_as(C.c_void_p), d.nbytes))
+        return dict(nx=int(d[0]), ny=int(d[1]), nz=int(d[2]), S=int(d[3]), nf=int(d[4]), cj=int(d[5]), ci=int(d[6]),
+                    bin_z=float(d[7:8].view(np.float32)[0]))
+
+    def mop_debug_get(self, what):
+        S = self.dims()["S"]
+        shape, dt = {"cell": ((self.nf, self.Q), np.int32), "perm": ((self.nf, S), np.int32),
+                     "xq": ((self.nf, S, 4), np.float32), "F": ((self.nf, self.Q, 3), np.float32),
+                     "eta": ((self.nf, self.Q, 3), np.float32), "Heta": ((self.nf, self.Q, 3), np.float32)}[what]
+        out = np.empty(shape, dt)
+        self._check(self.L.mop_debug_get(self.ctx, what.encode(), out.ctypes.data_as(C.c_void_p), out.nbytes))
+        return out
+
+    def mop_debug_pairs(self, bead, cap=None):
+        """Sorted (i<j) array of the in-range, non-excluded pairs of one force bead of the last evaluation."""
+        n = C.c_longlong(0)
+        if cap is None:
+            self._check(self.L.mop_debug_pairs(self.ctx, bead, None, 0, C.byref(n)))
+            cap = n.value
+        out = np.empty((max(cap, 1), 2), np.int32)
+        self._check(self.L.mop_debug_pairs(self.ctx, bead, out.ctypes.data_as(C.c_void_p), cap, C.byref(n)))
+        out = out[:min(cap, n.value)]
+        out = np.sort(out, axis=1)
+        order = np.lexsort((out[:, 1], out[:, 0]))
+        return out[order], int(n.value)
+
+    def mop_destroy(self):
+        if getattr(self, "ctx", None) is not None and self.ctx.value:
+            self.L.mop_destroy(self.ctx)
+            self.ctx = C.c_void_p()
+
+    close = mop_destroy
+
+    def __del__(self):
+        try:
+            self.mop_destroy()
+        except Exception:
+            pass

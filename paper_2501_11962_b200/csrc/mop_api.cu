@@ -1,0 +1,660 @@
+// mop_api.cu -- the C-ABI of include/mop.h: context, device memory, pass orchestration on one CUDA stream.
+// Every step of the hot path runs in the kernels of this directory; there is no CPU fallback.
+#include "../../include/mop.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "mop_bonded.cuh"
+#include "mop_common.cuh"
+#include "mop_grid.cuh"
+#include "mop_nonbonded.cuh"
+#include "mop_pairlist.cuh"
+#include "mop_path.cuh"
+
+static thread_local char g_create_error[256] = "";
+
+struct mop_ctx {
+    mop_params p;
+    int Q, N, nf;
+    cudaStream_t st;
+    MopGrid g;
+    float bin_z;
+    float rl, rl2, rc2;
+    float krf, crf;
+    bool has_topology = false;
+    int sticky = MOP_OK;
+    std::string err;
+    double n_launches = 0, n_rebuilds = 0;
+    int sm_count = 148;
+    // topology (device)
+    int nt = 0, n_bonds = 0, n_angles = 0, max_excl = 0;
+    float *d_mass = 0, *d_inv_mass = 0, *d_charge = 0, *d_ai = 0, *d_Ki = 0, *d_tabs = 0;
+    float2 *d_tab = 0, *d_bond_par = 0, *d_angle_par = 0;
+    int *d_type_row = 0, *d_bond_ij = 0, *d_angle_ijk = 0, *d_excl_start = 0, *d_excl_list = 0;
+    // per-bead sorted state
+    int *d_cell = 0, *d_cell_count = 0, *d_cell_rel = 0, *d_cell_fill = 0, *d_col_count = 0, *d_col_start = 0;
+    int *d_tmp = 0, *d_perm = 0, *d_slot_of = 0, *d_typ = 0;
+    float4 *d_xq = 0, *d_et = 0, *d_F4 = 0, *d_H4 = 0, *d_jlo = 0, *d_jhi = 0, *d_ilo = 0, *d_ihi = 0;
+    // pair list
+    MopUnit *d_units = 0;
+    MopEntry *d_entries = 0;
+    unsigned *d_masks = 0;
+    unsigned cap_units = 0, cap_entries = 0, cap_masks = 0;
+    MopCounters *d_ctr = 0;
+    unsigned long long *d_slots = 0;
+    unsigned *d_work = 0;   // [8]
+    double *d_energy = 0;   // [8]: U_lj, U_coul, U_bond, U_angle, E_spring, E_kin
+    // host mirrors (pinned)
+    double *h_energy = 0;
+    MopCounters *h_ctr = 0;
+    unsigned long long *h_slots = 0;
+    // scratch
+    float *d_G = 0;     // [N][Q][3] gradient for mop_step
+    float *d_dbg = 0;   // [nf][Q][3]
+    int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
+    double last_veff = 0, last_ekin = 0;
+};
+
+#define FAIL(c, code, ...)                                   \
+    do {                                                     \
+        char _b[256];                                        \
+        snprintf(_b, sizeof _b, __VA_ARGS__);                \
+        (c)->err = _b;                                       \
+        return (code);                                       \
+    } while (0)
+
+#define CK(c, call)                                                                                   \
+    do {                                                                                              \
+        cudaError_t _e = (call);                                                                      \
+        if (_e != cudaSuccess) {                                                                      \
+            (c)->sticky = (_e == cudaErrorMemoryAllocation) ? MOP_ERR_OOM : MOP_ERR_CUDA;             \
+            char _b[256];                                                                             \
+            snprintf(_b, sizeof _b, "%s at %s:%d: %s", #call, __FILE__, __LINE__, cudaGetErrorString(_e)); \
+            (c)->err = _b;                                                                            \
+            return (mop_status)(c)->sticky;                                                           \
+        }                                                                                             \
+    } while (0)
+
+#define LAUNCH(c, kernel, grid, block, smem, ...)                 \
+    do {                                                          \
+        kernel<<<(grid), (block), (smem), (c)->st>>>(__VA_ARGS__); \
+        (c)->n_launches += 1;                                     \
+    } while (0)
+
+template <typename T>
+static cudaError_t dalloc(T **p, size_t n) {
+    if (*p) {
+        cudaFree(*p);
+        *p = nullptr;
+    }
+    if (n == 0) n = 1;
+    return cudaMalloc((void **)p, n * sizeof(T));
+}
+
+static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_str() : g_create_error; }
+
+static void free_all(mop_ctx *c) {
+    void *ptrs[] = {c->d_mass,    c->d_inv_mass, c->d_charge,    c->d_ai,        c->d_Ki,       c->d_tabs,
+                    c->d_tab,     c->d_bond_par, c->d_angle_par, c->d_type_row,  c->d_bond_ij,  c->d_angle_ijk,
+                    c->d_excl_start, c->d_excl_list, c->d_cell,  c->d_cell_count, c->d_cell_rel, c->d_cell_fill,
+                    c->d_col_count, c->d_col_start, c->d_tmp,    c->d_perm,      c->d_slot_of,  c->d_typ,
+                    c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
+                    c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
+                    c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    if (c->h_energy) cudaFreeHost(c->h_energy);
+    if (c->h_ctr) cudaFreeHost(c->h_ctr);
+    if (c->h_slots) cudaFreeHost(c->h_slots);
+}
+
+extern "C" void mop_destroy(mop_ctx *c) {
+    if (!c) return;
+    cudaSetDevice(c->p.device);
+    cudaStreamSynchronize(c->st);
+    free_all(c);
+    delete c;
+}
+
+extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
+    if (!out || !p) {
+        snprintf(g_create_error, sizeof g_create_error, "mop_create: NULL argument");
+        return MOP_ERR_INVALID_ARG;
+    }
+    *out = nullptr;
+    auto bad = [&](mop_status s, const char *msg) {
+        snprintf(g_create_error, sizeof g_create_error, "mop_create: %s", msg);
+        return s;
+    };
+    if (p->n_atoms < 1 || p->n_beads < 1) return bad(MOP_ERR_INVALID_ARG, "n_atoms and n_beads must be >= 1");
+    if (!(p->r_cut > 0.f) || !(p->r_buf >= 0.f)) return bad(MOP_ERR_INVALID_ARG, "need r_cut > 0 and r_buf >= 0");
+    if (!(p->dt_path > 0.0) || !(p->nu > 0.0)) return bad(MOP_ERR_INVALID_ARG, "need dt_path > 0 and nu > 0");
+    for (int d = 0; d < 3; d++)
+        if (!(p->box[d] > 0.f) || !std::isfinite(p->box[d])) return bad(MOP_ERR_INVALID_ARG, "box must be positive");
+    const float rl = p->r_cut + p->r_buf;
+    for (int d = 0; d < 3; d++)
+        if (p->box[d] < 2.0f * rl) return bad(MOP_ERR_BOX_TOO_SMALL, "min(box) < 2 (r_cut + r_buf)");
+    if ((double)p->n_atoms * (double)p->n_beads > 1.0e9) return bad(MOP_ERR_INVALID_ARG, "n_atoms * n_beads too large");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || p->device < 0 || p->device >= ndev) {
+        cudaGetLastError();
+        return bad(MOP_ERR_CUDA, "no usable CUDA device (the library has no CPU fallback)");
+    }
+    if (cudaSetDevice(p->device) != cudaSuccess) return bad(MOP_ERR_CUDA, "cudaSetDevice failed");
+
+    mop_ctx *c = new mop_ctx();
+    c->p = *p;
+    c->Q = p->n_atoms;
+    c->N = p->n_beads;
+    c->nf = p->n_beads > 1 ? p->n_beads - 1 : 1;
+    c->st = (cudaStream_t)p->stream;
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    c->rl = rl;
+    c->rl2 = rl * rl * 1.0001f;
+    c->rc2 = p->r_cut * p->r_cut; // FP32 product (G8)
+    {
+        double rc = (double)p->r_cut;
+        double krf = p->eps_rf > 0.f ? ((double)p->eps_rf - 1.0) / ((2.0 * (double)p->eps_rf + 1.0) * rc * rc * rc)
+                                      : 1.0 / (2.0 * rc * rc * rc);
+        c->krf = (float)krf;
+        c->crf = (float)(1.0 / rc + krf * rc * rc);
+    }
+    // search grid (S0): columns of side ~ (32/rho)^(1/3) in x,y; thin bins of side/12 along z
+    MopGrid &g = c->g;
+    {
+        double vol = (double)p->box[0] * (double)p->box[1] * (double)p->box[2];
+        double side = cbrt((double)MOP_CJ * vol / (double)c->Q);
+        for (int d = 0; d < 2; d++) {
+            int n = (int)floor((double)p->box[d] / side);
+            g.dims[d] = n < 1 ? 1 : (n > 1024 ? 1024 : n);
+        }
+        c->bin_z = (float)(side / 12.0);
+        int nz = (int)floor((double)p->box[2] / (double)c->bin_z);
+        g.dims[2] = nz < 1 ? 1 : (nz > 4096 ? 4096 : nz);
+        for (int d = 0; d < 3; d++) {
+            g.box[d] = p->box[d];
+            g.inv_box[d] = 1.0f / p->box[d];
+            g.sc[d] = (float)g.dims[d] * g.inv_box[d];
+        }
+        g.ncol = g.dims[0] * g.dims[1];
+        g.ncell = g.ncol * g.dims[2];
+        g.colw[0] = p->box[0] / (float)g.dims[0];
+        g.colw[1] = p->box[1] / (float)g.dims[1];
+        g.Q = c->Q;
+        g.nf = c->nf;
+        size_t S = (size_t)c->Q + 31u * (size_t)g.ncol;
+        g.S = (int)((S + 31) / 32 * 32);
+    }
+    const size_t nf = c->nf, Q = c->Q, S = g.S;
+    cudaError_t e = cudaSuccess;
+    auto A = [&](cudaError_t r) {
+        if (e == cudaSuccess) e = r;
+    };
+    A(dalloc(&c->d_cell, nf * Q));
+    A(dalloc(&c->d_cell_count, nf * g.ncell));
+    A(dalloc(&c->d_cell_rel, nf * g.ncell));
+    A(dalloc(&c->d_cell_fill, nf * g.ncell));
+    A(dalloc(&c->d_col_count, nf * g.ncol));
+    A(dalloc(&c->d_col_start, nf * (g.ncol + 1)));
+    A(dalloc(&c->d_tmp, nf * S));
+    A(dalloc(&c->d_perm, nf * S));
+    A(dalloc(&c->d_slot_of, nf * Q));
+    A(dalloc(&c->d_typ, nf * S));
+    A(dalloc(&c->d_xq, nf * S));
+    A(dalloc(&c->d_et, nf * S));
+    A(dalloc(&c->d_F4, nf * S));
+    A(dalloc(&c->d_H4, nf * S));
+    A(dalloc(&c->d_jlo, nf * S / MOP_CJ));
+    A(dalloc(&c->d_jhi, nf * S / MOP_CJ));
+    A(dalloc(&c->d_ilo, nf * S / MOP_CI));
+    A(dalloc(&c->d_ihi, nf * S / MOP_CI));
+    A(dalloc(&c->d_ctr, 1));
+    A(dalloc(&c->d_slots, 1));
+    A(dalloc(&c->d_work, 8));
+    A(dalloc(&c->d_energy, 8));
+    A(cudaMallocHost((void **)&c->h_energy, 8 * sizeof(double)));
+    A(cudaMallocHost((void **)&c->h_ctr, sizeof(MopCounters)));
+    A(cudaMallocHost((void **)&c->h_slots, sizeof(unsigned long long)));
+    if (e != cudaSuccess) {
+        snprintf(g_create_error, sizeof g_create_error, "mop_create: device allocation failed: %s",
+                 cudaGetErrorString(e));
+        free_all(c);
+        delete c;
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? MOP_ERR_OOM : MOP_ERR_CUDA;
+    }
+    cudaMemsetAsync(c->d_energy, 0, 8 * sizeof(double), c->st);
+    cudaMemsetAsync(c->d_ctr, 0, sizeof(MopCounters), c->st);
+    cudaMemsetAsync(c->d_slots, 0, sizeof(unsigned long long), c->st);
+    memset(c->h_energy, 0, 8 * sizeof(double));
+    memset(c->h_ctr, 0, sizeof(MopCounters));
+    *c->h_slots = 0;
+    *out = c;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
+    if (!c) return MOP_ERR_INVALID_ARG;
+    if (c->sticky) return (mop_status)c->sticky;
+    if (!t || !t->mass || !t->charge || !t->type || !t->c6 || !t->c12) FAIL(c, MOP_ERR_INVALID_ARG, "NULL topology array");
+    const int Q = c->Q;
+    if (t->n_types < 1 || t->n_types > MOP_MAX_TYPES) FAIL(c, MOP_ERR_INVALID_ARG, "n_types must be in [1,%d]", MOP_MAX_TYPES);
+    if (t->n_bonds < 0 || t->n_angles < 0) FAIL(c, MOP_ERR_INVALID_ARG, "negative term count");
+    if ((t->n_bonds > 0 && (!t->bond_ij || !t->bond_b0_kb)) || (t->n_angles > 0 && (!t->angle_ijk || !t->angle_t0_kt)))
+        FAIL(c, MOP_ERR_INVALID_ARG, "NULL bonded array");
+    const int nt = t->n_types;
+    for (int i = 0; i < Q; i++) {
+        if (!(t->mass[i] > 0.f) || !std::isfinite(t->mass[i])) FAIL(c, MOP_ERR_INVALID_ARG, "mass[%d] must be > 0", i);
+        if (!std::isfinite(t->charge[i])) FAIL(c, MOP_ERR_INVALID_ARG, "charge[%d] not finite", i);
+        if (t->type[i] < 0 || t->type[i] >= nt) FAIL(c, MOP_ERR_INVALID_ARG, "type[%d] out of range", i);
+    }
+    for (int a = 0; a < nt; a++)
+        for (int b = 0; b < nt; b++)
+            if (t->c6[a * nt + b] != t->c6[b * nt + a] || t->c12[a * nt + b] != t->c12[b * nt + a])
+                FAIL(c, MOP_ERR_INVALID_ARG, "c6/c12 table not symmetric at (%d,%d)", a, b);
+    for (int b = 0; b < t->n_bonds; b++) {
+        int i = t->bond_ij[2 * b], j = t->bond_ij[2 * b + 1];
+        if (i < 0 || i >= Q || j < 0 || j >= Q || i == j) FAIL(c, MOP_ERR_INVALID_ARG, "bond %d: bad atom index", b);
+    }
+    for (int a = 0; a < t->n_angles; a++) {
+        int i = t->angle_ijk[3 * a], j = t->angle_ijk[3 * a + 1], k = t->angle_ijk[3 * a + 2];
+        if (i < 0 || i >= Q || j < 0 || j >= Q || k < 0 || k >= Q || i == j || j == k || i == k)
+            FAIL(c, MOP_ERR_INVALID_ARG, "angle %d: bad atom index", a);
+    }
+    int n_excl = 0, max_excl = 0;
+    if (t->excl_start) {
+        if (t->excl_start[0] != 0) FAIL(c, MOP_ERR_INVALID_ARG, "excl_start[0] != 0");
+        for (int i = 0; i < Q; i++)
+            if (t->excl_start[i + 1] < t->excl_start[i]) FAIL(c, MOP_ERR_INVALID_ARG, "excl_start not monotone at %d", i);
+        n_excl = t->excl_start[Q];
+        if (n_excl > 0 && !t->excl_list) FAIL(c, MOP_ERR_INVALID_ARG, "excl_list is NULL");
+        for (int i = 0; i < Q; i++) {
+            int e0 = t->excl_start[i], e1 = t->excl_start[i + 1];
+            if (e1 - e0 > max_excl) max_excl = e1 - e0;
+            for (int e = e0; e < e1; e++) {
+                int j = t->excl_list[e];
+                if (j < 0 || j >= Q || j == i) FAIL(c, MOP_ERR_INVALID_ARG, "exclusion of atom %d: bad partner", i);
+                if (e > e0 && t->excl_list[e - 1] >= j) FAIL(c, MOP_ERR_INVALID_ARG, "exclusions of atom %d not sorted", i);
+                // symmetric: i must be in j's list (binary search)
+                int lo = t->excl_start[j], hi = t->excl_start[j + 1] - 1;
+                bool found = false;
+                while (lo <= hi) {
+                    int mid = (lo + hi) / 2;
+                    int v = t->excl_list[mid];
+                    if (v == i) {
+                        found = true;
+                        break;
+                    }
+                    if (v < i) lo = mid + 1;
+                    else hi = mid - 1;
+                }
+                if (!found) FAIL(c, MOP_ERR_INVALID_ARG, "exclusion (%d,%d) not symmetric", i, j);
+            }
+        }
+    }
+    CK(c, cudaSetDevice(c->p.device));
+    c->nt = nt;
+    c->n_bonds = t->n_bonds;
+    c->n_angles = t->n_angles;
+    c->max_excl = max_excl;
+    // derived host arrays
+    std::vector<float> inv_m(Q), ai(Q), Ki(Q), tabs(nt * nt);
+    std::vector<int> trow(Q);
+    std::vector<float2> tab(nt * nt);
+    for (int i = 0; i < Q; i++) {
+        double m = (double)t->mass[i];
+        inv_m[i] = (float)(1.0 / m);
+        ai[i] = (float)(c->p.dt_path / (m * c->p.nu));       // L^n_i = a_i F^n_i  (G1)
+        Ki[i] = (float)(m * c->p.nu / (2.0 * c->p.dt_path));
+        trow[i] = t->type[i] * nt;
+    }
+    const double rc = (double)c->p.r_cut, irc6 = 1.0 / (rc * rc * rc * rc * rc * rc);
+    for (int k = 0; k < nt * nt; k++) {
+        tab[k] = make_float2(6.0f * t->c6[k], 12.0f * t->c12[k]);
+        tabs[k] = c->p.lj_shift ? (float)((double)t->c12[k] * irc6 * irc6 - (double)t->c6[k] * irc6) : 0.0f;
+    }
+    auto up = [&](auto **dst, const void *src, size_t n, size_t esz) -> cudaError_t {
+        cudaError_t r = dalloc(dst, n);
+        if (r != cudaSuccess) return r;
+        if (n == 0) return cudaSuccess;
+        return cudaMemcpyAsync(*dst, src, n * esz, cudaMemcpyHostToDevice, c->st);
+    };
+    CK(c, up(&c->d_mass, t->mass, Q, 4));
+    CK(c, up(&c->d_inv_mass, inv_m.data(), Q, 4));
+    CK(c, up(&c->d_charge, t->charge, Q, 4));
+    CK(c, up(&c->d_ai, ai.data(), Q, 4));
+    CK(c, up(&c->d_Ki, Ki.data(), Q, 4));
+    CK(c, up(&c->d_type_row, trow.data(), Q, 4));
+    CK(c, up(&c->d_tab, tab.data(), (size_t)nt * nt, 8));
+    CK(c, up(&c->d_tabs, tabs.data(), (size_t)nt * nt, 4));
+    CK(c, up(&c->d_bond_ij, t->bond_ij, (size_t)2 * t->n_bonds, 4));
+    CK(c, up(&c->d_bond_par, t->bond_b0_kb, (size_t)t->n_bonds, 8));
+    CK(c, up(&c->d_angle_ijk, t->angle_ijk, (size_t)3 * t->n_angles, 4));
+    CK(c, up(&c->d_angle_par, t->angle_t0_kt, (size_t)t->n_angles, 8));
+    if (t->excl_start && n_excl > 0) {
+        CK(c, up(&c->d_excl_start, t->excl_start, (size_t)Q + 1, 4));
+        CK(c, up(&c->d_excl_list, t->excl_list, (size_t)n_excl, 4));
+    } else {
+        if (c->d_excl_start) cudaFree(c->d_excl_start), c->d_excl_start = nullptr;
+        if (c->d_excl_list) cudaFree(c->d_excl_list), c->d_excl_list = nullptr;
+    }
+    // pair-list capacities (S1): volume bound on cluster pairs per i-cluster, with head room
+    {
+        const MopGrid &g = c->g;
+        double vol = (double)g.box[0] * g.box[1] * g.box[2];
+        double side = cbrt((double)MOP_CJ * vol / (double)Q);
+        double reach = 2.0 * c->rl + 2.0 * side;
+        double per_ci = 0.5 * ((double)Q / MOP_CJ / vol) * reach * reach * reach * 1.3;
+        if (per_ci < 64.0) per_ci = 64.0;
+        double nci = (double)c->nf * g.S / MOP_CI;
+        double ce = nci * per_ci;
+        if (ce > 3.5e9) ce = 3.5e9;
+        c->cap_entries = (unsigned)ce;
+        bool tiny = false;
+        for (int d = 0; d < 3; d++)
+            if (g.box[d] < 4.0f * c->rl) tiny = true;
+        double cu = nci * (tiny ? 27.0 : 4.0);
+        if (cu > 3.5e9) cu = 3.5e9;
+        c->cap_units = (unsigned)cu;
+        int rows = 1 + (max_excl > 0 ? std::min(12, 2 * max_excl + 2) : 0);
+        double cm = nci * rows;
+        if (cm > 3.5e9) cm = 3.5e9;
+        c->cap_masks = (unsigned)cm;
+        CK(c, dalloc(&c->d_units, (size_t)c->cap_units));
+        CK(c, dalloc(&c->d_entries, (size_t)c->cap_entries));
+        CK(c, dalloc(&c->d_masks, (size_t)c->cap_masks * MOP_CI));
+    }
+    // launch geometry of the persistent pair kernels
+    {
+        size_t smem = (size_t)nt * nt * 12;
+        CK(c, cudaFuncSetAttribute(k_nonbonded<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(c, cudaFuncSetAttribute(k_nonbonded<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CK(c, cudaFuncSetAttribute(k_nonbonded<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int b = 0;
+        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<false, false>, 128, smem));
+        c->nb_blocks_f = std::max(1, b) * c->sm_count;
+        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<false, true>, 128, smem));
+        c->nb_blocks_fe = std::max(1, b) * c->sm_count;
+        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<true, false>, 128, smem));
+        c->nb_blocks_h = std::max(1, b) * c->sm_count;
+    }
+    CK(c, cudaStreamSynchronize(c->st));
+    c->has_topology = true;
+    return MOP_OK;
+}
+
+// ---- S0 + S1 for the first nb beads of R ----
+static mop_status build_list(mop_ctx *c, const float *R, int nb) {
+    const MopGrid &g = c->g;
+    const size_t Q = c->Q;
+    CK(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
+    CK(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
+    CK(c, cudaMemsetAsync(c->d_ctr, 0, sizeof(MopCounters), c->st));
+    CK(c, cudaMemsetAsync(c->d_slots, 0, sizeof(unsigned long long), c->st));
+    dim3 ga(cdiv(Q, 256), nb), gs(cdiv(g.S, 256), nb);
+    LAUNCH(c, k_bin, ga, 256, 0, R, g, c->d_cell, c->d_cell_count);
+    LAUNCH(c, k_colscan, dim3(cdiv(g.ncol, 4), nb), 128, 0, g, c->d_cell_count, c->d_cell_rel, c->d_col_count);
+    LAUNCH(c, k_colstart, nb, 1024, 0, g, c->d_col_count, c->d_col_start);
+    LAUNCH(c, k_fill_pad, gs, 256, 0, g, c->d_perm, c->d_xq, c->d_typ);
+    LAUNCH(c, k_place, ga, 256, 0, g, c->d_cell, c->d_cell_rel, c->d_col_start, c->d_cell_fill, c->d_tmp);
+    LAUNCH(c, k_rank, ga, 256, 0, R, g, c->d_cell, c->d_cell_rel, c->d_col_start, c->d_cell_count, c->d_tmp,
+           c->d_charge, c->d_type_row, c->d_perm, c->d_slot_of, c->d_xq, c->d_typ);
+    LAUNCH(c, k_bbox, dim3(cdiv(g.S / MOP_CJ, 4), nb), 128, 0, g, c->d_perm, c->d_xq, c->d_jlo, c->d_jhi, c->d_ilo,
+           c->d_ihi);
+    PlArgs a;
+    a.g = g;
+    a.rl = c->rl;
+    a.rl2 = c->rl2;
+    a.perm = c->d_perm, a.slot_of = c->d_slot_of, a.xq = c->d_xq;
+    a.jlo = c->d_jlo, a.jhi = c->d_jhi, a.ilo = c->d_ilo, a.ihi = c->d_ihi;
+    a.col_start = c->d_col_start;
+    a.excl_start = c->d_excl_start, a.excl_list = c->d_excl_list;
+    a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
+    a.slots_active = c->d_slots;
+    a.cap_units = c->cap_units, a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks;
+    const unsigned nci_blocks = cdiv(g.S / MOP_CI, 4);
+    a.bead0 = 0;
+    LAUNCH(c, k_pairlist, dim3(nci_blocks, 1), 128, 0, a); // bead 1 first: its units come first (energy variant)
+    LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr);
+    if (nb > 1) {
+        a.bead0 = 1;
+        LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 128, 0, a);
+    }
+    c->n_rebuilds += 1;
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+static const auto kfe = k_nonbonded<false, true>;
+static const auto kf = k_nonbonded<false, false>;
+static const auto kh = k_nonbonded<true, false>;
+
+static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
+    NbArgs a;
+    a.S = c->g.S, a.nt = c->nt;
+    a.rc2 = c->rc2;
+    a.k2rf = 2.0f * c->krf, a.krf = c->krf, a.crf = c->crf;
+    a.xq = c->d_xq, a.typ = c->d_typ, a.et = c->d_et, a.out = out;
+    a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
+    a.work = c->d_work + work_slot;
+    a.range = range;
+    a.tab = c->d_tab, a.tabs = c->d_tabs;
+    a.energies = c->d_energy;
+    for (int d = 0; d < 3; d++) a.box[d] = c->g.box[d];
+    return a;
+}
+
+static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
+    BondedArgs b;
+    b.Q = c->Q, b.S = c->g.S, b.n_bonds = c->n_bonds, b.n_angles = c->n_angles;
+    b.R = R, b.slot_of = c->d_slot_of;
+    b.bond_ij = c->d_bond_ij, b.bond_par = c->d_bond_par, b.angle_ijk = c->d_angle_ijk, b.angle_par = c->d_angle_par;
+    b.et = c->d_et, b.out = out, b.energies = c->d_energy;
+    for (int d = 0; d < 3; d++) b.box[d] = c->g.box[d], b.inv_box[d] = c->g.inv_box[d];
+    return b;
+}
+
+// pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded
+static mop_status pass_force(mop_ctx *c, const float *R, int nb) {
+    const size_t smem = (size_t)c->nt * c->nt * 12;
+    CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
+    LAUNCH(c, kfe, c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
+    if (nb > 1) LAUNCH(c, kf, c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    const int nterm = c->n_bonds + c->n_angles;
+    if (nterm > 0) LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_F4));
+    return MOP_OK;
+}
+
+// pass 2 on the first nb beads: nonbonded + bonded Hessian-vector product with the direction held in et
+static mop_status pass_hvp(mop_ctx *c, const float *R, int nb) {
+    const size_t smem = (size_t)c->nt * c->nt * 12;
+    CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
+    LAUNCH(c, kh, c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
+    const int nterm = c->n_bonds + c->n_angles;
+    if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));
+    return MOP_OK;
+}
+
+static mop_status read_back(mop_ctx *c) {
+    CK(c, cudaMemcpyAsync(c->h_energy, c->d_energy, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaMemcpyAsync(c->h_slots, c->d_slots, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    CK(c, cudaGetLastError());
+    if (c->h_ctr->overflow) {
+        c->sticky = MOP_ERR_OOM;
+        FAIL(c, MOP_ERR_OOM, "pair-list buffer overflow (flags 0x%x: 1 entries, 2 units, 4 masks, 8 staging, 16 excl rows)",
+             c->h_ctr->overflow);
+    }
+    const double *E = c->h_energy;
+    c->last_veff = E[0] + E[1] + E[2] + E[3] + E[4];
+    c->last_ekin = E[5];
+    if (!std::isfinite(c->last_veff)) FAIL(c, MOP_ERR_NONFINITE, "V_eff is not finite (overlapping atoms?)");
+    return MOP_OK;
+}
+
+static mop_status eval_async(mop_ctx *c, const float *R, float *grad) {
+    const int nb = c->nf;
+    CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
+    CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    mop_status s = build_list(c, R, nb);
+    if (s) return s;
+    if ((s = pass_force(c, R, nb))) return s;
+    if (c->N > 1) {
+        LAUNCH(c, k_eta, dim3(cdiv(c->g.S, 256), nb), 256, 0, c->Q, c->g.S, R, c->d_perm, c->d_typ, c->d_F4, c->d_ai,
+               c->d_Ki, c->d_et, c->d_energy + 4);
+        if ((s = pass_hvp(c, R, nb))) return s;
+    }
+    if (grad)
+        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->d_slot_of, c->d_F4, c->d_et,
+               c->d_H4, c->d_Ki, grad);
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+#define PRECHECK(c)                                                          \
+    do {                                                                     \
+        if (!(c)) return MOP_ERR_INVALID_ARG;                                \
+        if ((c)->sticky) return (mop_status)(c)->sticky;                     \
+        if (!(c)->has_topology) FAIL(c, MOP_ERR_NO_TOPOLOGY, "call mop_set_topology first"); \
+        CK(c, cudaSetDevice((c)->p.device));                                 \
+    } while (0)
+
+extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double *veff_out, float *grad_dev) {
+    PRECHECK(c);
+    if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
+    mop_status s = eval_async(c, R_dev, grad_dev);
+    if (s) return s;
+    if (veff_out) {
+        if ((s = read_back(c))) return s;
+        *veff_out = c->last_veff;
+    }
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps) {
+    PRECHECK(c);
+    if (!R_dev || !V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or V_dev is NULL");
+    if (n_steps < 0 || !(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
+    const size_t total = (size_t)c->N * c->Q * 3;
+    if (!c->d_G) CK(c, dalloc(&c->d_G, total));
+    mop_status s = eval_async(c, R_dev, c->d_G);
+    if (s) return s;
+    const unsigned nblk = cdiv(total, 256);
+    for (int it = 0; it < n_steps; it++) {
+        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
+               (double *)nullptr);
+        if ((s = eval_async(c, R_dev, c->d_G))) return s;
+        const bool last = it == n_steps - 1;
+        if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
+        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
+               last ? c->d_energy + 5 : (double *)nullptr);
+    }
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_get_stats(mop_ctx *c, double out[16]) {
+    PRECHECK(c);
+    if (!out) FAIL(c, MOP_ERR_INVALID_ARG, "out is NULL");
+    mop_status s = read_back(c);
+    if (s && s != MOP_ERR_NONFINITE) return s;
+    const double *E = c->h_energy;
+    out[0] = c->last_veff;
+    out[1] = E[0] + E[1] + E[2] + E[3];
+    out[2] = E[4];
+    out[3] = E[0], out[4] = E[1], out[5] = E[2], out[6] = E[3];
+    out[7] = E[5];
+    out[8] = c->n_rebuilds;
+    out[9] = (double)c->h_ctr->n_entries;
+    out[10] = (double)c->h_ctr->n_units;
+    out[11] = (double)c->h_ctr->n_masks;
+    out[12] = (double)(*c->h_slots) * 32.0;
+    out[13] = c->n_launches;
+    out[14] = out[15] = 0.0;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_debug_get(mop_ctx *c, const char *what, void *host_buf, size_t bytes) {
+    PRECHECK(c);
+    if (!what || !host_buf) FAIL(c, MOP_ERR_INVALID_ARG, "NULL argument");
+    const MopGrid &g = c->g;
+    const size_t nf = c->nf, Q = c->Q, S = g.S;
+    std::string w(what);
+    auto copy = [&](const void *src, size_t n) -> mop_status {
+        if (bytes != n) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_get(%s): expected %zu bytes, got %zu", what, n, bytes);
+        CK(c, cudaMemcpyAsync(host_buf, src, n, cudaMemcpyDeviceToHost, c->st));
+        CK(c, cudaStreamSynchronize(c->st));
+        return MOP_OK;
+    };
+    if (w == "dims") {
+        int d[8] = {g.dims[0], g.dims[1], g.dims[2], g.S, c->nf, MOP_CJ, MOP_CI, 0};
+        memcpy(&d[7], &c->bin_z, 4);
+        if (bytes != sizeof d) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_get(dims): expected %zu bytes", sizeof d);
+        memcpy(host_buf, d, sizeof d);
+        return MOP_OK;
+    }
+    if (w == "cell") return copy(c->d_cell, nf * Q * 4);
+    if (w == "perm") return copy(c->d_perm, nf * S * 4);
+    if (w == "xq") return copy(c->d_xq, nf * S * 16);
+    const float4 *src = nullptr;
+    if (w == "F") src = c->d_F4;
+    else if (w == "eta") src = c->d_et;
+    else if (w == "Heta") src = c->d_H4;
+    else FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_get: unknown array '%s'", what);
+    if (!c->d_dbg) CK(c, dalloc(&c->d_dbg, nf * Q * 3));
+    LAUNCH(c, k_gather3, dim3(cdiv(Q, 256), (unsigned)nf), 256, 0, c->Q, g.S, c->d_slot_of, src, c->d_dbg, 1.0f);
+    return copy(c->d_dbg, nf * Q * 12);
+}
+
+extern "C" mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long long cap, long long *n_pairs) {
+    PRECHECK(c);
+    if (bead < 0 || bead >= c->nf || !n_pairs || cap < 0 || (cap > 0 && !pairs))
+        FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_pairs: bad argument");
+    int *d_pairs = nullptr;
+    CK(c, dalloc(&d_pairs, (size_t)2 * cap));
+    PairDbgArgs a;
+    a.S = c->g.S, a.bead = bead, a.rc2 = c->rc2;
+    a.xq = c->d_xq, a.perm = c->d_perm, a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks;
+    a.ctr = c->d_ctr, a.pairs = d_pairs, a.cap = cap;
+    for (int d = 0; d < 3; d++) a.box[d] = c->g.box[d];
+    cudaMemsetAsync(&c->d_ctr->n_pairs, 0, sizeof(unsigned long long), c->st);
+    LAUNCH(c, k_debug_pairs, c->sm_count * 8, 128, 0, a);
+    cudaError_t e = cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    if (e == cudaSuccess) {
+        *n_pairs = (long long)c->h_ctr->n_pairs;
+        long long ncopy = std::min(*n_pairs, cap);
+        if (ncopy > 0) e = cudaMemcpy(pairs, d_pairs, (size_t)ncopy * 8, cudaMemcpyDeviceToHost);
+    }
+    cudaFree(d_pairs);
+    CK(c, e);
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float *s_dev, float *F_dev, float *Hs_dev) {
+    PRECHECK(c);
+    if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
+    if (Hs_dev && !s_dev) FAIL(c, MOP_ERR_INVALID_ARG, "Hs_dev needs s_dev");
+    CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
+    CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    mop_status s = build_list(c, R_dev, 1);
+    if (s) return s;
+    if ((s = pass_force(c, R_dev, 1))) return s;
+    const MopGrid &g = c->g;
+    if (F_dev) LAUNCH(c, k_gather3, dim3(cdiv(c->Q, 256), 1), 256, 0, c->Q, g.S, c->d_slot_of, c->d_F4, F_dev, 1.0f);
+    if (Hs_dev) {
+        LAUNCH(c, k_set_dir, cdiv(g.S, 256), 256, 0, g.S, c->d_perm, c->d_typ, s_dev, c->d_et);
+        if ((s = pass_hvp(c, R_dev, 1))) return s;
+        LAUNCH(c, k_gather3, dim3(cdiv(c->Q, 256), 1), 256, 0, c->Q, g.S, c->d_slot_of, c->d_H4, Hs_dev, 1.0f);
+    }
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}

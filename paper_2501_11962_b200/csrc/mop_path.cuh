@@ -1,0 +1,123 @@
+// mop_path.cuh -- S4 (displacements eta^n and spring energy: the paper's PMD kernels 1 and 7),
+// S7 (gradient assembly: PMD kernels 4-6, eqs (5),(6),(7)) and S8 (velocity Verlet on
+// eq. (4)).  Elementwise, HBM-bound.
+#pragma once
+#include "mop_common.cuh"
+
+// eta^n_i = (R^{n+1}_i - R^n_i) - a_i F^n_i,  a_i = dt/(m_i nu)  (L^n = a F^n, reading G1)
+// E_spring += K_i/2 |eta^n_i|^2, K_i = m_i nu/(2 dt), accumulated in FP64.  One thread per sorted slot.
+__global__ void __launch_bounds__(256) k_eta(int Q, int S, const float *__restrict__ R,
+                                             const int *__restrict__ perm, const int *__restrict__ typ,
+                                             const float4 *__restrict__ F4, const float *__restrict__ a_i,
+                                             const float *__restrict__ K_i, float4 *__restrict__ et,
+                                             double *__restrict__ e_spring) {
+    const int n = blockIdx.y;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (s < S) {
+        const size_t o = (size_t)n * S + s;
+        const int i = perm[o];
+        float4 out = make_float4(0.f, 0.f, 0.f, __int_as_float(typ[o]));
+        if (i >= 0) {
+            const float *r0 = R + ((size_t)n * Q + i) * 3, *r1 = r0 + (size_t)Q * 3;
+            const float4 f = F4[o];
+            const float a = a_i[i];
+            out.x = __fmaf_rn(-a, f.x, r1[0] - r0[0]);
+            out.y = __fmaf_rn(-a, f.y, r1[1] - r0[1]);
+            out.z = __fmaf_rn(-a, f.z, r1[2] - r0[2]);
+            e = 0.5 * (double)K_i[i] *
+                ((double)out.x * (double)out.x + (double)out.y * (double)out.y + (double)out.z * (double)out.z);
+        }
+        et[o] = out;
+    }
+    __shared__ double sh[8];
+    e = mop_warp_sum_d(e);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = e;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+        v = mop_warp_sum_d(v);
+        if (threadIdx.x == 0 && v != 0.0) atomicAdd(e_spring, v);
+    }
+}
+
+// dV_eff/dR^n_i (= -F_eff of eqs 5,6,7 with the bracket at its eps->0 limit -1/2 H eta):
+//   n = 1     : -F^1 - K eta^1 + 1/2 H^1 eta^1          (N = 1: -F^1)
+//   1 < n < N : K eta^{n-1} - K eta^n + 1/2 H^n eta^n
+//   n = N     : K eta^{N-1}
+__global__ void __launch_bounds__(256) k_assemble(int Q, int S, int N, const int *__restrict__ slot_of,
+                                                  const float4 *__restrict__ F4, const float4 *__restrict__ et,
+                                                  const float4 *__restrict__ H4, const float *__restrict__ K_i,
+                                                  float *__restrict__ grad) {
+    const int n = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Q) return;
+    float gx = 0.f, gy = 0.f, gz = 0.f;
+    const float K = K_i[i];
+    if (n == 0) {
+        const float4 f = F4[slot_of[i]];
+        gx -= f.x, gy -= f.y, gz -= f.z;
+    }
+    if (n > 0) {
+        const float4 e = et[(size_t)(n - 1) * S + slot_of[(size_t)(n - 1) * Q + i]];
+        gx = fmaf(K, e.x, gx), gy = fmaf(K, e.y, gy), gz = fmaf(K, e.z, gz);
+    }
+    if (n < N - 1) {
+        const size_t o = (size_t)n * S + slot_of[(size_t)n * Q + i];
+        const float4 e = et[o], h = H4[o];
+        gx += fmaf(-K, e.x, 0.5f * h.x), gy += fmaf(-K, e.y, 0.5f * h.y), gz += fmaf(-K, e.z, 0.5f * h.z);
+    }
+    float *g = grad + ((size_t)n * Q + i) * 3;
+    g[0] = gx, g[1] = gy, g[2] = gz;
+}
+
+// sorted float4 array -> original-order [nf][Q][3]
+__global__ void __launch_bounds__(256) k_gather3(int Q, int S, const int *__restrict__ slot_of,
+                                                 const float4 *__restrict__ src, float *__restrict__ dst,
+                                                 float scale) {
+    const int n = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Q) return;
+    const float4 v = src[(size_t)n * S + slot_of[(size_t)n * Q + i]];
+    float *d = dst + ((size_t)n * Q + i) * 3;
+    d[0] = scale * v.x, d[1] = scale * v.y, d[2] = scale * v.z;
+}
+
+// user direction s [Q][3] -> et of bead slot 0 (mop_force_hvp)
+__global__ void __launch_bounds__(256) k_set_dir(int S, const int *__restrict__ perm, const int *__restrict__ typ,
+                                                 const float *__restrict__ sdir, float4 *__restrict__ et) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const int i = perm[s];
+    float4 out = make_float4(0.f, 0.f, 0.f, __int_as_float(typ[s]));
+    if (i >= 0) out.x = sdir[3 * (size_t)i], out.y = sdir[3 * (size_t)i + 1], out.z = sdir[3 * (size_t)i + 2];
+    et[s] = out;
+}
+
+// velocity Verlet: mode 0  v += (dt/2)(-G)/m ; R += dt v      mode 1  v += (dt/2)(-G)/m (+ kinetic energy)
+__global__ void __launch_bounds__(256) k_verlet(size_t total, int Q, float dt, int mode, const float *__restrict__ inv_m,
+                                                const float *__restrict__ m, const float *__restrict__ G,
+                                                float *__restrict__ R, float *__restrict__ V,
+                                                double *__restrict__ e_kin) {
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double ek = 0.0;
+    if (o < total) {
+        const int i = (int)((o / 3) % (size_t)Q);
+        float v = V[o];
+        v = fmaf(-0.5f * dt * inv_m[i], G[o], v);
+        V[o] = v;
+        if (mode == 0) R[o] = fmaf(dt, v, R[o]);
+        else if (e_kin) ek = 0.5 * (double)m[i] * (double)v * (double)v;
+    }
+    if (mode == 1 && e_kin) {
+        __shared__ double sh[8];
+        ek = mop_warp_sum_d(ek);
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = ek;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            double v = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+            v = mop_warp_sum_d(v);
+            if (threadIdx.x == 0) atomicAdd(e_kin, v);
+        }
+    }
+}

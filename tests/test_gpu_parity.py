@@ -1,0 +1,269 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the FP64 oracle, element by element, on the
+same seeded inputs.  Bars (BASELINE.json north_star): neighbour sets bit-exact, V_eff relative error <= 1e-6,
+RMS relative error (G14) <= 1e-4 for forces and gradient.  All tests here need a B200 (-m gpu).
+"""
+import numpy as np
+import pytest
+
+from paper_2501_11962_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+TOL_V = 1e-6
+TOL_RMS = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device: the library has no CPU fallback")
+    from paper_2501_11962_b200 import binding
+    binding.load()
+    return binding
+
+
+_CACHE = {}
+
+
+def case(oracle, name):
+    """(system, OracleSystem, path R float32 [N][Q][3]) for a named parity case (seeded, cached)."""
+    if name in _CACHE:
+        return _CACHE[name]
+    if name == "c1":
+        s = W.config1(n_beads=16)
+    elif name == "c2":
+        s = W.config2(n_beads=8)          # config 2 at N=8 (the N=64 form runs in test_config2_full)
+    elif name == "c2_full":
+        s = W.config2(n_beads=64)
+    elif name == "chain":
+        s = H.tiny_chain()
+        s.n_beads = 6
+    elif name == "c3":
+        s = W.config3(n_beads=3)
+    elif name == "memb":
+        s = W.small_membrane(n_beads=3)
+    elif name == "lj_n1":
+        s = W.config1(n_beads=1)
+    elif name == "lj_n2":
+        s = W.config1(n_beads=2)
+    else:
+        raise KeyError(name)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, s.n_beads, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    _CACHE[name] = (s, o, R)
+    return _CACHE[name]
+
+
+# --------------------------------------------------------------------------- S0: cell ids + stable sort
+@pytest.mark.parametrize("name", ["c1", "c2", "chain", "memb"])
+def test_cell_ids_and_stable_sort_bit_exact(B, oracle, name):
+    s, o, R = case(oracle, name)
+    m = B.Mop(s, s.n_beads)
+    m.mop_eval_veff_grad(R, want_grad=False)
+    d = m.dims()
+    dims = [d["nx"], d["ny"], d["nz"]]
+    assert dims == oracle.grid_dims(s.n_atoms, o.box, d["cj"], d["bin_z"])
+    cell = m.mop_debug_get("cell")
+    perm = m.mop_debug_get("perm")
+    xq = m.mop_debug_get("xq")
+    ncell = dims[0] * dims[1] * dims[2]
+    for n in range(m.nf):
+        xw = oracle.wrap(R[n], o.box)
+        c_ref = oracle.cell_ids(xw, o.box, dims)
+        assert np.array_equal(cell[n], c_ref), "cell ids differ on bead %d" % n
+        p_ref = oracle.stable_sort_by_cell(c_ref, ncell)
+        real = perm[n] >= 0
+        assert np.array_equal(perm[n][real], p_ref), "stable permutation differs on bead %d" % n
+        # sorted coordinates are the wrapped ones, bit for bit; charges ride along
+        assert np.array_equal(xq[n][real][:, :3], xw[p_ref])
+        assert np.array_equal(xq[n][real][:, 3], np.asarray(s.charge, np.float32)[p_ref])
+        # padding only at column ends: inside a column the real slots come first, columns start at multiples of 32
+        col = c_ref[p_ref] // dims[2]
+        slots = np.flatnonzero(real)
+        for cc in np.unique(col)[:50]:
+            sl = slots[col == cc]
+            assert sl[0] % 32 == 0 and np.array_equal(sl, np.arange(sl[0], sl[0] + len(sl)))
+    m.close()
+
+
+# --------------------------------------------------------------------------- O1: neighbour sets
+@pytest.mark.parametrize("name,brute", [("c1", True), ("c2", True), ("chain", True), ("c3", False), ("memb", False)])
+def test_neighbour_sets_bit_exact(B, oracle, name, brute):
+    s, o, R = case(oracle, name)
+    m = B.Mop(s, s.n_beads)
+    m.mop_eval_veff_grad(R, want_grad=False)
+    beads = range(m.nf) if s.n_atoms <= 3000 else [0, m.nf - 1]
+    for n in beads:
+        ref = oracle.pairs(o, R[n].astype(np.float64), geom=1, brute=brute)
+        got, cnt = m.mop_debug_pairs(n)
+        assert cnt == len(ref), "pair count differs on bead %d: %d vs %d" % (n, cnt, len(ref))
+        assert np.array_equal(got, ref), "pair set differs on bead %d" % n
+    m.close()
+
+
+# --------------------------------------------------------------------------- O2/O3: force and H.s of one bead
+@pytest.mark.parametrize("name", ["c1", "c2", "chain", "memb"])
+def test_force_and_hvp_single_bead(B, oracle, name):
+    s, o, R = case(oracle, name)
+    rng = np.random.default_rng(5)
+    sv = rng.normal(0, 1e-3, (s.n_atoms, 3)).astype(np.float32)
+    m = B.Mop(s, 1)
+    X = R[min(1, len(R) - 1)]
+    F, Hs = m.mop_force_hvp(X, sv)
+    ref = oracle.bead(o, X.astype(np.float64), geom=1, brute=s.n_atoms <= 3000, s=sv.astype(np.float64))
+    assert H.rms_rel(F.cpu().numpy(), ref["F"]) <= TOL_RMS
+    assert H.rms_rel(Hs.cpu().numpy(), ref["Hs"]) <= TOL_RMS
+    # invariants on the GPU output itself: Newton's third law (P6)
+    Fn = F.double().cpu().numpy()
+    assert np.abs(Fn.sum(0)).max() <= 1e-5 * np.abs(Fn).sum(0).max()
+    m.close()
+
+
+# --------------------------------------------------------------------------- O4/O5: V_eff and its gradient
+@pytest.mark.parametrize("name", ["c1", "c2", "chain", "c3", "memb", "lj_n1", "lj_n2"])
+def test_veff_and_gradient(B, oracle, name):
+    s, o, R = case(oracle, name)
+    m = B.Mop(s, s.n_beads)
+    v, g = m.mop_eval_veff_grad(R)
+    v_ref, g_ref, parts = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=s.n_atoms <= 3000, want_parts=True)
+    st = m.mop_get_stats()
+    # per stage, so that a failure localises
+    assert H.rms_rel(m.mop_debug_get("F"), parts["F"]) <= TOL_RMS
+    if s.n_beads > 1:
+        assert H.rms_rel(m.mop_debug_get("eta"), parts["eta"]) <= TOL_RMS
+        assert H.rms_rel(m.mop_debug_get("Heta"), parts["Heta"]) <= TOL_RMS
+    assert abs(st["U1"] - parts["U1"]) <= TOL_V * max(abs(parts["U1"]), abs(v_ref))
+    assert abs(st["E_spring"] - parts["E_spring"]) <= TOL_V * abs(v_ref)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    m.close()
+
+
+def test_config2_full_64_beads(B, oracle):
+    s, o, R = case(oracle, "c2_full")
+    m = B.Mop(s, 64)
+    v, g = m.mop_eval_veff_grad(R)
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=False)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    m.close()
+
+
+def test_async_eval_matches_sync_and_repeats(B, oracle):
+    """veff_out = NULL leaves the value in the context; repeated evaluations agree to float-atomic noise."""
+    s, o, R = case(oracle, "c2")
+    m = B.Mop(s, s.n_beads)
+    v1, g1 = m.mop_eval_veff_grad(R)
+    _, g2 = m.mop_eval_veff_grad(R, sync=False)
+    v2 = m.mop_get_stats()["veff"]
+    assert abs(v1 - v2) <= 1e-9 * abs(v1)
+    assert H.rms_rel(g2.cpu().numpy(), g1.cpu().numpy()) <= 1e-5
+    m.close()
+
+
+# --------------------------------------------------------------------------- O6: velocity Verlet
+@pytest.mark.parametrize("name", ["c1", "chain"])
+def test_step_matches_oracle(B, oracle, name):
+    import torch
+    s, o, R = case(oracle, name)
+    rng = np.random.default_rng(11)
+    sd = np.sqrt(W.KB * s.temperature / s.mass.astype(np.float64))
+    V0 = (rng.normal(0, 1, R.shape) * sd[None, :, None]).astype(np.float32)
+    m = B.Mop(s, s.n_beads)
+    Rg = torch.tensor(R, device="cuda")
+    Vg = torch.tensor(V0, device="cuda")
+    nst, dt = 5, 0.001
+    m.mop_step(Rg, Vg, dt, nst)
+    R_ref, V_ref, en = oracle.step(o, R.astype(np.float64), V0.astype(np.float64), dt, nst, geom=1, brute=True)
+    dR_ref = R_ref - R.astype(np.float64)
+    dR = Rg.cpu().numpy().astype(np.float64) - R.astype(np.float64)
+    # FP32 positions: each update rounds at ulp(R) ~ 2e-7 nm against displacements of ~5e-3 nm
+    assert H.rms_rel(dR, dR_ref) <= 2e-3
+    assert H.rms_rel(Vg.cpu().numpy(), V_ref) <= 1e-4
+    ek = m.mop_get_stats()["E_kin"]
+    assert abs(ek - en[-1, 1]) <= 1e-4 * en[-1, 1]
+    m.close()
+
+
+def test_nve_energy_conservation(B, oracle):
+    """Fig. 4a analogue: total energy V_eff + E_kin of the polymer is conserved by mop_step."""
+    import torch
+    s, o, R = case(oracle, "c1")
+    rng = np.random.default_rng(12)
+    sd = np.sqrt(W.KB * s.temperature / s.mass.astype(np.float64))
+    m = B.Mop(s, s.n_beads)
+    Rg = torch.tensor(R, device="cuda")
+    Vg = torch.tensor((rng.normal(0, 1, R.shape) * sd[None, :, None]).astype(np.float32), device="cuda")
+    tot = []
+    for _ in range(6):
+        m.mop_step(Rg, Vg, 0.0005, 20)
+        st = m.mop_get_stats()
+        tot.append(st["veff"] + st["E_kin"])
+    ekin = st["E_kin"]
+    assert max(tot) - min(tot) <= 2e-3 * ekin
+    m.close()
+
+
+# --------------------------------------------------------------------------- degenerate inputs and errors
+def test_edge_cases(B, oracle):
+    # two atoms, one pair; then out of range
+    for r, npair in ((0.5, 1), (1.05, 0)):
+        s = H.two_atoms(r, q=(0.3, -0.3), lj_shift=1)
+        o = oracle.OracleSystem(s)
+        m = B.Mop(s, 1)
+        v, g = m.mop_eval_veff_grad(s.R1[None].astype(np.float32))
+        v_ref, g_ref = oracle.veff_grad(o, s.R1[None].astype(np.float32).astype(np.float64), geom=1, brute=True)
+        assert m.mop_debug_pairs(0)[1] == npair
+        assert abs(v - v_ref) <= 1e-6 * max(abs(v_ref), 1e-3)
+        assert np.allclose(g.cpu().numpy(), g_ref, rtol=1e-4, atol=1e-4)
+        m.close()
+    # one atom: no pairs at all, zero energy and gradient
+    s = H.make_system("one", [3.0] * 3, [[1.0, 1.0, 1.0]], [12.0], [0.5], [0], [0.3], [0.5])
+    m = B.Mop(s, 3)
+    R = np.tile(np.float32(s.R1), (3, 1, 1)) + np.float32([[[0.0]], [[0.001]], [[0.003]]])
+    v, g = m.mop_eval_veff_grad(R)
+    K = 12.0 * 50.0 / (2 * 0.002)
+    assert v == pytest.approx(0.5 * K * 3 * (0.001 ** 2 + 0.002 ** 2), rel=1e-3)
+    m.close()
+
+
+def test_atoms_outside_the_box_and_on_faces(B, oracle):
+    """Caller coordinates are never wrapped per bead; atoms far outside [0,L) and exactly on faces."""
+    s, o, R = case(oracle, "c1")
+    R2 = R.copy()
+    R2[:, ::3, 0] += np.float32(2.88) * 3     # whole images away, consistently along the path
+    R2[:, 1::5, 1] -= np.float32(2.88) * 2
+    R2[0, 0] = [0.0, 2.88, 5.76]
+    R2[1:, 0] = R2[0, 0] + (R[1:, 0] - R[0, 0])
+    m = B.Mop(s, s.n_beads)
+    v, g = m.mop_eval_veff_grad(R2)
+    for n in (0, m.nf - 1):
+        ref = oracle.pairs(o, R2[n].astype(np.float64), geom=1, brute=True)
+        got, cnt = m.mop_debug_pairs(n)
+        assert cnt == len(ref) and np.array_equal(got, ref)
+    v_ref, g_ref = oracle.veff_grad(o, R2.astype(np.float64), geom=1, brute=True)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    m.close()
+
+
+def test_error_codes(B):
+    s = W.config1(n_beads=2)
+    s.box = np.asarray([1.9, 2.88, 2.88], np.float32)
+    with pytest.raises(B.MopError) as e:
+        B.Mop(s, 2)
+    assert e.value.status == 3
+    s = W.config1(n_beads=2)
+    s.mass = s.mass.copy()
+    s.mass[7] = 0.0
+    with pytest.raises(B.MopError) as e:
+        B.Mop(s, 2)
+    assert e.value.status == 1
+    s = W.config2(n_beads=2)
+    s.excl_list = s.excl_list.copy()
+    s.excl_list[0] = 5          # asymmetric exclusion
+    with pytest.raises(B.MopError) as e:
+        B.Mop(s, 2)
+    assert e.value.status == 1

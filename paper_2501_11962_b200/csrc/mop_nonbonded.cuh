@@ -31,6 +31,7 @@ struct NbArgs {
     unsigned *work;     // dynamic work counter (zeroed before the launch)
     int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all
     const float2 *tab;  // [nt*nt] (6 C6, 12 C12)
+    const float2 *tabe; // [nt*nt] (C6, C12) as given (energy: no rounding bias from the prefactors)
     const float *tabs;  // [nt*nt] LJ energy shift C12 rc^-12 - C6 rc^-6 (0 when lj_shift = 0)
     double *energies;   // [0] U_lj, [1] U_coul
     float box[3];
@@ -38,7 +39,8 @@ struct NbArgs {
 
 template <bool HVP, bool ENERGY, bool SHIFT>
 __device__ __forceinline__ void nb_unit(const NbArgs &a, const MopUnit &un, const float2 *__restrict__ tab,
-                                        const float *__restrict__ tabs, const int lane) {
+                                        const float2 *__restrict__ tabe, const float *__restrict__ tabs,
+                                        const int lane) {
     const size_t boff = (size_t)un.bead * a.S;
     const float4 *__restrict__ xq = a.xq + boff;
     const float4 *__restrict__ et = a.et + boff;
@@ -61,9 +63,9 @@ __device__ __forceinline__ void nb_unit(const NbArgs &a, const MopUnit &un, cons
         if (HVP) {
             float4 e = et[un.ci * MOP_CI + k];
             sxi[k] = e.x, syi[k] = e.y, szi[k] = e.z;
-            ri[k] = __float_as_int(e.w);
+            ri[k] = __float_as_int(e.w) * a.nt;
         } else {
-            ri[k] = typ[un.ci * MOP_CI + k];
+            ri[k] = typ[un.ci * MOP_CI + k] * a.nt;
         }
         ax[k] = ay[k] = az[k] = 0.f;
     }
@@ -100,6 +102,10 @@ __device__ __forceinline__ void nb_unit(const NbArgs &a, const MopUnit &un, cons
             const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
             const bool inr = (r2 < a.rc2) && allowed;
             float rinv = rsqrtf(r2);
+            if (ENERGY) { // one Newton step: removes the approximation's bias from the energy sum
+                const float er = __fmaf_rn(-__fmul_rn(r2, rinv), rinv, 1.0f);
+                rinv = __fmaf_rn(0.5f * rinv, er, rinv);
+            }
             rinv = inr ? rinv : 0.f;
             const float qq = inr ? qi[k] * cp.w : 0.f;
             const float2 cc = tab[ri[k] + ctj];
@@ -114,7 +120,8 @@ __device__ __forceinline__ void nb_unit(const NbArgs &a, const MopUnit &un, cons
                 jx = fmaf(g, dx, jx), jy = fmaf(g, dy, jy), jz = fmaf(g, dz, jz);
                 if (ENERGY) {
                     const float sh = inr ? tabs[ri[k] + ctj] : 0.f;
-                    u_lj += p12 * (1.0f / 12.0f) - p6 * (1.0f / 6.0f) - sh;
+                    const float2 ce6 = tabe[ri[k] + ctj];
+                    u_lj += __fmaf_rn(ce6.y * r6i, r6i, -__fmaf_rn(ce6.x, r6i, sh));
                     u_c += qq * (rinv + a.krf * r2 - a.crf);
                 }
             } else {
@@ -162,9 +169,11 @@ template <bool HVP, bool ENERGY>
 __global__ void __launch_bounds__(128) k_nonbonded(const NbArgs a) {
     extern __shared__ float4 s_dyn[];
     float2 *tab = reinterpret_cast<float2 *>(s_dyn);
-    float *tabs = reinterpret_cast<float *>(tab + a.nt * a.nt);
+    float2 *tabe = tab + a.nt * a.nt;
+    float *tabs = reinterpret_cast<float *>(tabe + a.nt * a.nt);
     for (int t = threadIdx.x; t < a.nt * a.nt; t += blockDim.x) {
         tab[t] = a.tab[t];
+        tabe[t] = a.tabe[t];
         tabs[t] = a.tabs[t];
     }
     __syncthreads();
@@ -183,8 +192,8 @@ __global__ void __launch_bounds__(128) k_nonbonded(const NbArgs a) {
         un.bead = (int)u0.x, un.ci = (int)u0.y, un.shift = (int)u0.z, un.start = u0.w;
         un.count = u1.x, un.excl_base = u1.y;
         if (un.count == 0) continue;
-        if (un.shift == 13) nb_unit<HVP, ENERGY, false>(a, un, tab, tabs, lane);
-        else nb_unit<HVP, ENERGY, true>(a, un, tab, tabs, lane);
+        if (un.shift == 13) nb_unit<HVP, ENERGY, false>(a, un, tab, tabe, tabs, lane);
+        else nb_unit<HVP, ENERGY, true>(a, un, tab, tabe, tabs, lane);
     }
 }
 

@@ -158,7 +158,7 @@ def test_async_eval_matches_sync_and_repeats(B, oracle):
     v1, g1 = m.mop_eval_veff_grad(R)
     _, g2 = m.mop_eval_veff_grad(R, sync=False)
     v2 = m.mop_get_stats()["veff"]
-    assert abs(v1 - v2) <= 1e-9 * abs(v1)
+    assert abs(v1 - v2) <= 1e-7 * abs(v1)   # float-atomic order noise in F -> eta -> E_spring
     assert H.rms_rel(g2.cpu().numpy(), g1.cpu().numpy()) <= 1e-5
     m.close()
 

@@ -100,6 +100,12 @@ mop_status mop_set_topology(mop_ctx *c, const mop_topology *t);
  * Errors: NO_TOPOLOGY, INVALID_ARG, OOM (list overflow, reported at a synchronising call), CUDA, NONFINITE. */
 mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double *veff_out, float *grad_dev);
 
+/* The same evaluation with HOST buffers (the end-to-end form): copies R_host [N][Q][3] to the device on the
+ * context stream, evaluates, copies the gradient back to grad_host [N][Q][3] (may be NULL) and V_eff to *veff_out
+ * (required).  Pinned host memory makes the copies asynchronous to the host until the final synchronisation;
+ * pageable memory works too.  Synchronises.  The device staging buffers belong to the context. */
+mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff_out, float *grad_host);
+
 /* n_steps velocity-Verlet steps of eq. (4) with F_eff = -grad V_eff and masses m_i, step dt_pmd (ps):
  *   v += dt/2 F_eff/m ; R += dt v ; F_eff(R) ; v += dt/2 F_eff/m.
  * R_dev, V_dev DEVICE [N][Q][3] float, updated in place.  The gradient at the incoming R is evaluated at the
@@ -120,6 +126,16 @@ const char *mop_last_error(const mop_ctx *c);
  * [12]=pair slots evaluated per nonbonded pass (entries * 8 * 32), [13]=kernel launches so far,
  * [14],[15] reserved. */
 mop_status mop_get_stats(mop_ctx *c, double out[16]);
+
+/* Stage timing with CUDA events on the context stream (the stream the kernels are launched on).  on != 0: every
+ * later mop_eval_veff_grad / _host / mop_step evaluation records 9 events around its stages; on or off: the
+ * accumulated sums are reset.  Evaluations made through mop_force_hvp are not timed. */
+mop_status mop_set_timing(mop_ctx *c, int on);
+
+/* Synchronises with the timed evaluations issued so far.  out[k], k = 0..7: mean milliseconds per evaluation of
+ * stage S0 grid build, S1 pair list, S2 nonbonded force kernels, S3 bonded force, S4 eta + spring energy,
+ * S5 nonbonded H.eta kernel, S6 bonded H.eta, S7 assembly; out[8] = evaluations averaged; rest 0. */
+mop_status mop_get_timing(mop_ctx *c, double out[16]);
 
 /* Copies an internal array of the last evaluation to HOST memory (synchronises).  `what`:
  *   "dims"  int[8]: nx, ny, nz (search grid), slots per bead S (padded, multiple of 32), force beads nf,

@@ -16,7 +16,8 @@ MOP_OK = 0
 STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "MOP_ERR_BOX_TOO_SMALL",
           4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
-           "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp"]
+           "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
+           "mop_set_timing", "mop_get_timing"]
 
 
 class MopError(RuntimeError):
@@ -68,8 +69,11 @@ def load(build_if_missing=True):
     L.mop_debug_get.argtypes = [C.c_void_p, C.c_char_p, C.c_void_p, C.c_size_t]
     L.mop_debug_pairs.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_longlong, C.POINTER(C.c_longlong)]
     L.mop_force_hvp.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.mop_eval_veff_grad_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+    L.mop_set_timing.argtypes = [C.c_void_p, C.c_int]
+    L.mop_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
-              "mop_debug_pairs", "mop_force_hvp"):
+              "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
         getattr(L, n).restype = C.c_int
     _lib = L
     return L
@@ -161,6 +165,30 @@ class Mop:
         self._check(self.L.mop_eval_veff_grad(self.ctx, _ptr(R), C.byref(v) if sync else None,
                                               _ptr(grad) if want_grad else None))
         return (v.value if sync else None), (grad if want_grad else None)
+
+    def mop_eval_veff_grad_host(self, R_host, grad_host=None):
+        """HOST buffers (torch CPU tensors, ideally pinned, float32 [N][Q][3]).  Returns V_eff; fills grad_host."""
+        assert not R_host.is_cuda and R_host.is_contiguous() and tuple(R_host.shape) == (self.N, self.Q, 3)
+        assert R_host.dtype == self.torch.float32
+        if grad_host is not None:
+            assert not grad_host.is_cuda and grad_host.is_contiguous() and grad_host.shape == R_host.shape
+            assert grad_host.dtype == self.torch.float32
+        v = C.c_double(0.0)
+        self._check(self.L.mop_eval_veff_grad_host(self.ctx, _ptr(R_host), C.byref(v), _ptr(grad_host)))
+        return v.value
+
+    def mop_set_timing(self, on):
+        self._check(self.L.mop_set_timing(self.ctx, int(bool(on))))
+
+    def mop_get_timing(self):
+        """Mean ms per evaluation of each stage since mop_set_timing, and the number of evaluations averaged."""
+        out = (C.c_double * 16)()
+        self._check(self.L.mop_get_timing(self.ctx, out))
+        k = ["S0_grid", "S1_pairlist", "S2_nb_force", "S3_bonded_force", "S4_eta", "S5_nb_hvp", "S6_bonded_hvp",
+             "S7_assemble"]
+        d = dict(zip(k, list(out)[:8]))
+        d["evals"] = int(out[8])
+        return d
 
     def mop_step(self, R, V, dt_pmd, n_steps):
         """In-place velocity Verlet on torch cuda tensors R, V [N][Q][3] float32."""

@@ -18,6 +18,9 @@
 
 static thread_local char g_create_error[256] = "";
 
+#define MOP_NSTAGE 8  // S0 grid, S1 pair list, S2 nonbonded force, S3 bonded force, S4 eta, S5 nonbonded H.eta, S6 bonded H.eta, S7 assembly
+#define MOP_TSETS 64
+
 struct mop_ctx {
     mop_params p;
     int Q, N, nf;
@@ -58,6 +61,14 @@ struct mop_ctx {
     float *d_dbg = 0;   // [nf][Q][3]
     int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
     double last_veff = 0, last_ekin = 0;
+    // e2e staging (mop_eval_veff_grad_host)
+    float *d_Rh = 0, *d_Gh = 0;
+    // stage timing (mop_set_timing): a ring of event sets, one per evaluation
+    bool timing = false;
+    cudaEvent_t ev[MOP_TSETS][MOP_NSTAGE + 1];
+    bool ev_made = false;
+    int ev_head = 0, ev_pending = 0;   // sets [head-pending, head) await collection
+    double t_sum[MOP_NSTAGE] = {0}, t_cnt = 0;
 };
 
 #define FAIL(c, code, ...)                                   \
@@ -107,12 +118,16 @@ static void free_all(mop_ctx *c) {
                     c->d_col_count, c->d_col_start, c->d_tmp,    c->d_perm,      c->d_slot_of,  c->d_typ,
                     c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
                     c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
-                    c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg};
+                    c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg,       c->d_Rh,
+                    c->d_Gh};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (c->h_energy) cudaFreeHost(c->h_energy);
     if (c->h_ctr) cudaFreeHost(c->h_ctr);
     if (c->h_slots) cudaFreeHost(c->h_slots);
+    if (c->ev_made)
+        for (auto &set : c->ev)
+            for (cudaEvent_t e : set) cudaEventDestroy(e);
 }
 
 extern "C" void mop_destroy(mop_ctx *c) {
@@ -392,8 +407,31 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     return MOP_OK;
 }
 
+// ---- stage timing: event k closes stage k-1 of the evaluation in flight (no-ops unless mop_set_timing(1)) ----
+static void t_collect(mop_ctx *c, int n_sets) {
+    // oldest first; blocks the host until those evaluations have finished
+    for (; n_sets > 0 && c->ev_pending > 0; n_sets--, c->ev_pending--) {
+        const int set = ((c->ev_head - c->ev_pending) % MOP_TSETS + MOP_TSETS) % MOP_TSETS;
+        if (cudaEventSynchronize(c->ev[set][MOP_NSTAGE]) != cudaSuccess) continue;
+        for (int k = 0; k < MOP_NSTAGE; k++) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, c->ev[set][k], c->ev[set][k + 1]) == cudaSuccess) c->t_sum[k] += (double)ms;
+        }
+        c->t_cnt += 1;
+    }
+}
+static void t_mark(mop_ctx *c, int k) {
+    if (!c->timing) return;
+    if (k == 0 && c->ev_pending == MOP_TSETS) t_collect(c, 1);
+    cudaEventRecord(c->ev[c->ev_head % MOP_TSETS][k], c->st);
+    if (k == MOP_NSTAGE) {
+        c->ev_head = (c->ev_head + 1) % MOP_TSETS;
+        c->ev_pending += 1;
+    }
+}
+
 // ---- S0 + S1 for the first nb beads of R ----
-static mop_status build_list(mop_ctx *c, const float *R, int nb) {
+static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = false) {
     const MopGrid &g = c->g;
     const size_t Q = c->Q;
     CK(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
@@ -410,6 +448,7 @@ static mop_status build_list(mop_ctx *c, const float *R, int nb) {
            c->d_charge, c->d_type_row, c->d_perm, c->d_slot_of, c->d_xq, c->d_typ);
     LAUNCH(c, k_bbox, dim3(cdiv(g.S / MOP_CJ, 4), nb), 128, 0, g, c->d_perm, c->d_xq, c->d_jlo, c->d_jhi, c->d_ilo,
            c->d_ihi);
+    if (timed) t_mark(c, 1);
     PlArgs a;
     a.g = g;
     a.rl = c->rl;
@@ -430,6 +469,7 @@ static mop_status build_list(mop_ctx *c, const float *R, int nb) {
         LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 128, 0, a);
     }
     c->n_rebuilds += 1;
+    if (timed) t_mark(c, 2);
     CK(c, cudaGetLastError());
     return MOP_OK;
 }
@@ -464,23 +504,27 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
 }
 
 // pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded
-static mop_status pass_force(mop_ctx *c, const float *R, int nb) {
+static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false) {
     const size_t smem = (size_t)c->nt * c->nt * 20;
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
     LAUNCH(c, kfe, c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
     if (nb > 1) LAUNCH(c, kf, c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    if (timed) t_mark(c, 3);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_F4));
+    if (timed) t_mark(c, 4);
     return MOP_OK;
 }
 
 // pass 2 on the first nb beads: nonbonded + bonded Hessian-vector product with the direction held in et
-static mop_status pass_hvp(mop_ctx *c, const float *R, int nb) {
+static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = false) {
     const size_t smem = (size_t)c->nt * c->nt * 20;
     CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
     LAUNCH(c, kh, c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
+    if (timed) t_mark(c, 6);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));
+    if (timed) t_mark(c, 7);
     return MOP_OK;
 }
 
@@ -506,17 +550,22 @@ static mop_status eval_async(mop_ctx *c, const float *R, float *grad) {
     const int nb = c->nf;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
-    mop_status s = build_list(c, R, nb);
+    t_mark(c, 0);
+    mop_status s = build_list(c, R, nb, true);
     if (s) return s;
-    if ((s = pass_force(c, R, nb))) return s;
+    if ((s = pass_force(c, R, nb, true))) return s;
     if (c->N > 1) {
         LAUNCH(c, k_eta, dim3(cdiv(c->g.S, 256), nb), 256, 0, c->Q, c->g.S, R, c->d_perm, c->d_typ, c->d_F4, c->d_ai,
                c->d_Ki, c->d_et, c->d_energy + 4);
-        if ((s = pass_hvp(c, R, nb))) return s;
+        t_mark(c, 5);
+        if ((s = pass_hvp(c, R, nb, true))) return s;
+    } else {
+        t_mark(c, 5), t_mark(c, 6), t_mark(c, 7);
     }
     if (grad)
         LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->d_slot_of, c->d_F4, c->d_et,
                c->d_H4, c->d_Ki, grad);
+    t_mark(c, 8);
     CK(c, cudaGetLastError());
     return MOP_OK;
 }
@@ -538,6 +587,48 @@ extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double 
         if ((s = read_back(c))) return s;
         *veff_out = c->last_veff;
     }
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff_out, float *grad_host) {
+    PRECHECK(c);
+    if (!R_host || !veff_out) FAIL(c, MOP_ERR_INVALID_ARG, "R_host or veff_out is NULL");
+    const size_t bytes = (size_t)c->N * c->Q * 3 * sizeof(float);
+    if (!c->d_Rh) CK(c, dalloc(&c->d_Rh, (size_t)c->N * c->Q * 3));
+    if (grad_host && !c->d_Gh) CK(c, dalloc(&c->d_Gh, (size_t)c->N * c->Q * 3));
+    CK(c, cudaMemcpyAsync(c->d_Rh, R_host, bytes, cudaMemcpyHostToDevice, c->st));
+    mop_status s = eval_async(c, c->d_Rh, grad_host ? c->d_Gh : nullptr);
+    if (s) return s;
+    if (grad_host) CK(c, cudaMemcpyAsync(grad_host, c->d_Gh, bytes, cudaMemcpyDeviceToHost, c->st));
+    if ((s = read_back(c))) return s;
+    *veff_out = c->last_veff;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_set_timing(mop_ctx *c, int on) {
+    if (!c) return MOP_ERR_INVALID_ARG;
+    if (c->sticky) return (mop_status)c->sticky;
+    CK(c, cudaSetDevice(c->p.device));
+    if (on && !c->ev_made) {
+        for (auto &set : c->ev)
+            for (cudaEvent_t &e : set) CK(c, cudaEventCreate(&e));
+        c->ev_made = true;
+    }
+    if (c->ev_made) t_collect(c, MOP_TSETS);
+    c->timing = on != 0;
+    for (double &t : c->t_sum) t = 0.0;
+    c->t_cnt = 0;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_get_timing(mop_ctx *c, double out[16]) {
+    if (!c || !out) return MOP_ERR_INVALID_ARG;
+    if (c->sticky) return (mop_status)c->sticky;
+    CK(c, cudaSetDevice(c->p.device));
+    if (c->ev_made) t_collect(c, MOP_TSETS);
+    for (int k = 0; k < 16; k++) out[k] = 0.0;
+    for (int k = 0; k < MOP_NSTAGE; k++) out[k] = c->t_cnt > 0 ? c->t_sum[k] / c->t_cnt : 0.0;
+    out[8] = c->t_cnt;
     return MOP_OK;
 }
 

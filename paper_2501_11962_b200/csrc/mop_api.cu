@@ -60,6 +60,7 @@ struct mop_ctx {
     float *d_G = 0;     // [N][Q][3] gradient for mop_step
     float *d_dbg = 0;   // [nf][Q][3]
     int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
+    int var_f = 0, var_h = 0;   // tuning variants of the pair kernels (NBV_* flags)
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
@@ -108,6 +109,14 @@ static cudaError_t dalloc(T **p, size_t n) {
 }
 
 static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
+
+typedef void (*nb_kernel_t)(const NbArgs);
+#define NB_VARIANTS(MODE)                                                                                         \
+    {k_nonbonded<MODE, 0>, k_nonbonded<MODE, 1>, k_nonbonded<MODE, 2>, k_nonbonded<MODE, 3>, k_nonbonded<MODE, 4>, \
+     k_nonbonded<MODE, 5>, k_nonbonded<MODE, 6>, k_nonbonded<MODE, 7>}
+static const nb_kernel_t k_force[8] = NB_VARIANTS(NB_FORCE);
+static const nb_kernel_t k_energy[8] = NB_VARIANTS(NB_ENERGY);
+static const nb_kernel_t k_hvp[8] = NB_VARIANTS(NB_HVP);
 
 extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_str() : g_create_error; }
 
@@ -390,17 +399,18 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     }
     // launch geometry of the persistent pair kernels
     {
-        size_t smem = (size_t)nt * nt * 20;
-        CK(c, cudaFuncSetAttribute(k_nonbonded<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(c, cudaFuncSetAttribute(k_nonbonded<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CK(c, cudaFuncSetAttribute(k_nonbonded<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int b = 0;
-        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<false, false>, 128, smem));
-        c->nb_blocks_f = std::max(1, b) * c->sm_count;
-        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<false, true>, 128, smem));
-        c->nb_blocks_fe = std::max(1, b) * c->sm_count;
-        CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_nonbonded<true, false>, 128, smem));
-        c->nb_blocks_h = std::max(1, b) * c->sm_count;
+        const size_t smem = nb_smem_bytes(nt);
+        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 7;
+        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 7;
+        const void *fns[3] = {(const void *)k_force[c->var_f], (const void *)k_energy[c->var_f],
+                              (const void *)k_hvp[c->var_h]};
+        int *nbs[3] = {&c->nb_blocks_f, &c->nb_blocks_fe, &c->nb_blocks_h};
+        for (int k = 0; k < 3; k++) {
+            CK(c, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int b = 0;
+            CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, fns[k], 128, smem));
+            *nbs[k] = std::max(1, b) * c->sm_count;
+        }
     }
     CK(c, cudaStreamSynchronize(c->st));
     c->has_topology = true;
@@ -474,9 +484,6 @@ static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = fa
     return MOP_OK;
 }
 
-static const auto kfe = k_nonbonded<false, true>;
-static const auto kf = k_nonbonded<false, false>;
-static const auto kh = k_nonbonded<true, false>;
 
 static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     NbArgs a;
@@ -505,10 +512,10 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
 
 // pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded
 static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false) {
-    const size_t smem = (size_t)c->nt * c->nt * 20;
+    const size_t smem = nb_smem_bytes(c->nt);
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, kfe, c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
-    if (nb > 1) LAUNCH(c, kf, c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    LAUNCH(c, k_energy[c->var_f], c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
+    if (nb > 1) LAUNCH(c, k_force[c->var_f], c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
     if (timed) t_mark(c, 3);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_F4));
@@ -518,9 +525,9 @@ static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = fa
 
 // pass 2 on the first nb beads: nonbonded + bonded Hessian-vector product with the direction held in et
 static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = false) {
-    const size_t smem = (size_t)c->nt * c->nt * 20;
+    const size_t smem = nb_smem_bytes(c->nt);
     CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, kh, c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
+    LAUNCH(c, k_hvp[c->var_h], c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
     if (timed) t_mark(c, 6);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));

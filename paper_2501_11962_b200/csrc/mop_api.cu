@@ -13,6 +13,7 @@
 #include "mop_common.cuh"
 #include "mop_grid.cuh"
 #include "mop_nonbonded.cuh"
+#include "mop_nonbonded_packed.cuh"
 #include "mop_pairlist.cuh"
 #include "mop_path.cuh"
 
@@ -60,7 +61,7 @@ struct mop_ctx {
     float *d_G = 0;     // [N][Q][3] gradient for mop_step
     float *d_dbg = 0;   // [nf][Q][3]
     int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
-    int var_f = 0, var_h = 0;   // tuning variants of the pair kernels (NBV_* flags)
+    int var_f = 8, var_h = 8;   // tuning variants of the pair kernels (NBV_* flags)
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
@@ -117,6 +118,18 @@ typedef void (*nb_kernel_t)(const NbArgs);
 static const nb_kernel_t k_force[8] = NB_VARIANTS(NB_FORCE);
 static const nb_kernel_t k_energy[8] = NB_VARIANTS(NB_ENERGY);
 static const nb_kernel_t k_hvp[8] = NB_VARIANTS(NB_HVP);
+// variants 8..15: the packed (f32x2) kernels, NBP_* flags in the low three bits
+#define NBP_VARIANTS(MODE)                                                                                    \
+    {k_nonbonded_p<MODE, 0>, k_nonbonded_p<MODE, 1>, k_nonbonded_p<MODE, 2>, k_nonbonded_p<MODE, 3>,          \
+     k_nonbonded_p<MODE, 4>, k_nonbonded_p<MODE, 5>, k_nonbonded_p<MODE, 6>, k_nonbonded_p<MODE, 7>}
+static const nb_kernel_t k_force_p[8] = NBP_VARIANTS(NB_FORCE);
+static const nb_kernel_t k_energy_p[8] = NBP_VARIANTS(NB_ENERGY);
+static const nb_kernel_t k_hvp_p[8] = NBP_VARIANTS(NB_HVP);
+static size_t nb_smem(const mop_ctx *c, int var) { return var >= 8 ? nbp_smem_bytes(c->nt) : nb_smem_bytes(c->nt); }
+static nb_kernel_t nb_pick(int mode, int var) {
+    if (var >= 8) return (mode == NB_FORCE ? k_force_p : mode == NB_ENERGY ? k_energy_p : k_hvp_p)[var & 7];
+    return (mode == NB_FORCE ? k_force : mode == NB_ENERGY ? k_energy : k_hvp)[var & 7];
+}
 
 extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_str() : g_create_error; }
 
@@ -399,13 +412,13 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     }
     // launch geometry of the persistent pair kernels
     {
-        const size_t smem = nb_smem_bytes(nt);
-        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 7;
-        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 7;
-        const void *fns[3] = {(const void *)k_force[c->var_f], (const void *)k_energy[c->var_f],
-                              (const void *)k_hvp[c->var_h]};
+        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 15;
+        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 15;
+        const void *fns[3] = {(const void *)nb_pick(NB_FORCE, c->var_f), (const void *)nb_pick(NB_ENERGY, c->var_f),
+                              (const void *)nb_pick(NB_HVP, c->var_h)};
         int *nbs[3] = {&c->nb_blocks_f, &c->nb_blocks_fe, &c->nb_blocks_h};
         for (int k = 0; k < 3; k++) {
+            const size_t smem = nb_smem(c, k == 2 ? c->var_h : c->var_f);
             CK(c, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             int b = 0;
             CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, fns[k], 128, smem));
@@ -465,7 +478,7 @@ static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = fa
     a.rl2 = c->rl2;
     a.perm = c->d_perm, a.slot_of = c->d_slot_of, a.xq = c->d_xq;
     a.jlo = c->d_jlo, a.jhi = c->d_jhi, a.ilo = c->d_ilo, a.ihi = c->d_ihi;
-    a.col_start = c->d_col_start;
+    a.col_start = c->d_col_start, a.cell_rel = c->d_cell_rel, a.col_count = c->d_col_count;
     a.excl_start = c->d_excl_start, a.excl_list = c->d_excl_list;
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.slots_active = c->d_slots;
@@ -512,10 +525,10 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
 
 // pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded
 static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false) {
-    const size_t smem = nb_smem_bytes(c->nt);
+    const size_t smem = nb_smem(c, c->var_f);
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, k_energy[c->var_f], c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
-    if (nb > 1) LAUNCH(c, k_force[c->var_f], c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    LAUNCH(c, nb_pick(NB_ENERGY, c->var_f), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
+    if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
     if (timed) t_mark(c, 3);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_F4));
@@ -525,9 +538,9 @@ static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = fa
 
 // pass 2 on the first nb beads: nonbonded + bonded Hessian-vector product with the direction held in et
 static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = false) {
-    const size_t smem = nb_smem_bytes(c->nt);
+    const size_t smem = nb_smem(c, c->var_h);
     CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, k_hvp[c->var_h], c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
+    LAUNCH(c, nb_pick(NB_HVP, c->var_h), c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
     if (timed) t_mark(c, 6);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));

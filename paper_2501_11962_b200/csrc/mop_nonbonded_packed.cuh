@@ -1,0 +1,380 @@
+// mop_nonbonded_packed.cuh -- the production form of S2 (pass 1: force, energy on bead 1) and S5 (pass 2: fused
+// force-scalar + Hessian-vector pair kernel), SURVEY.md 8a.  FP32-pipe-bound; no tensor cores.
+#pragma once
+#include "mop_nonbonded.cuh"
+
+// =====================================================================================================
+// Packed variant: two i atoms per lane per issue slot (sm_100a FFMA2 / FMUL2 / FADD2 = fma|mul|add.rn.f32x2).
+// The pair kernels are bound by issue slots when written with scalar FP32 instructions (profiles/r01_ncu_summary.md);
+// the packed form halves the FP issue count, which leaves the FP32 pipe itself (128 lanes/clk/SM) as the bound.
+// Lane l still owns atom l of the current j-cluster; a packed register holds the same quantity for i atoms
+// (2p, 2p+1), p = 0..3.  All packed operations are IEEE round-to-nearest per component, so the G8 predicate
+// (d = xs_i - xw_j, r2 = fma(dz,dz,fma(dy,dy,dx*dx)), r2 < rc*rc) is bit-identical to the scalar form.
+// Sign conventions chosen so that no negation is needed in the row body:
+//   gn = -g = x (B - A) + C - 2 k_rf ke qi qj,      hn = -h = x (x (8A - 14B) - 3C),      dn = s_j - s_i = -delta
+//   F_i += gn d;                (H s)_i += hn (d.dn) d + gn dn;        the j side accumulates the same sums (jn),
+//   and the lane's j atom receives -(jn.lo + jn.hi) once per entry.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 f2_pack(float lo, float hi) {
+    f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(f2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f2 f2_bc(float s) { return f2_pack(s, s); }
+__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
+    f2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ void f2_acc(f2 &c, f2 a, f2 b) { // c += a * b, in place
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ f2 f2_mul(f2 a, f2 b) {
+    f2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
+    f2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f2 f2_sub(f2 a, f2 b) {
+    f2 d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// staging reads are volatile so that the compiler re-reads shared memory per entry instead of pinning the
+// eight i atoms in registers for the whole unit
+__device__ __forceinline__ float4 mop_lds_v4(unsigned addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float2 mop_lds_v2(unsigned addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float mop_lds_f(unsigned addr) {
+    float v;
+    asm("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ unsigned mop_lds_vu(unsigned addr) {
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint2 mop_lds_vu2(unsigned addr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+// asynchronous global -> shared copies (LDGSTS): the j atoms of the entries ahead are in flight while one is processed
+__device__ __forceinline__ void mop_cp_async16(unsigned saddr, const void *g) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void mop_cp_async4(unsigned saddr, const void *g) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void mop_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void mop_cp_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
+       NBP_OCC6 = 4 };  // ask for 6 resident CTAs per SM (register cap 80)
+#define NBP_NST 4       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1)
+
+// Shared memory of one CTA (4 warps), bytes:
+//   [0, 1024)              i-atom staging, 256 B per warp: for p = 0..3 at float offset 16 p
+//                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
+//   [1024, 2048)           the current chunk of up to 32 list entries, 256 B per warp
+//   [2048, 2048 + 16 KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
+//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), (C6, C12)[nt*nt] as given, energy shift [nt*nt]
+#define NBP_SM_ENT 1024u
+#define NBP_SM_RING 2048u
+#define NBP_SM_TAB (2048u + 4u * NBP_NST * 1024u)
+__host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 20; }
+
+template <int MODE, int VAR>
+__device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, float *__restrict__ sw,
+                                         const unsigned sw_addr, const unsigned se_addr, const unsigned sr_addr,
+                                         const unsigned tab6, const unsigned off12,
+                                         const float2 *__restrict__ tabe, const float *__restrict__ tabs,
+                                         const int lane) {
+    constexpr bool HVP = MODE == NB_HVP, ENERGY = MODE == NB_ENERGY;
+    const unsigned boff = (unsigned)un.bead * (unsigned)a.S; // nf * S < 2^31 (checked at create)
+    const float4 *__restrict__ xq = a.xq + boff;
+    const float4 *__restrict__ et = a.et + boff;
+    const int *__restrict__ typ = a.typ + boff;
+    float4 *__restrict__ out = a.out + boff;
+
+    __syncwarp();
+    if (lane < MOP_CI) {
+        float sx, sy, sz;
+        mop_unit_shift(un.shift, a.box, sx, sy, sz);
+        float4 p = xq[un.ci * MOP_CI + lane];
+        float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
+        int ti;
+        if (HVP) {
+            e = et[un.ci * MOP_CI + lane];
+            ti = __float_as_int(e.w);
+        } else {
+            ti = typ[un.ci * MOP_CI + lane];
+        }
+        float *d = sw + (lane >> 1) * 16 + (lane & 1);
+        d[0] = __fsub_rn(p.x, sx), d[2] = __fsub_rn(p.y, sy), d[4] = __fsub_rn(p.z, sz);
+        d[6] = p.w * MOP_KE;
+        d[8] = e.x, d[10] = e.y, d[12] = e.z;
+        d[14] = __int_as_float((int)tab6 + ti * a.nt * 4);
+    }
+    __syncwarp();
+
+    f2 ax[4], ay[4], az[4];
+#pragma unroll
+    for (int p = 0; p < 4; p++) ax[p] = ay[p] = az[p] = 0ull;
+    double e_lj = 0.0, e_c = 0.0;
+    const f2 nk2rf = f2_bc(-a.k2rf);
+    const unsigned lane16 = (unsigned)lane * 16u;
+
+    // one entry: the 32 j atoms (cp, ce, type offset tj4) against the 8 i atoms.
+    // Phase L (branch-free, four independent chains): d, r2 and the G8 test for all four packed row pairs.
+    // Phase H: the pair math for the row pairs in which some lane is in range (warp votes).
+    auto entry = [&](const uint2 cur, const float4 cp, const float4 ce, const unsigned tj4) {
+        const f2 jx = f2_bc(cp.x), jy = f2_bc(cp.y), jz = f2_bc(cp.z), jq = f2_bc(cp.w);
+        f2 r2v[4];
+        bool anyp[4];
+#pragma unroll
+        for (int p = 0; p < 4; p++) {
+            const float4 P0 = mop_lds_v4(sw_addr + p * 64);
+            const float2 P1 = mop_lds_v2(sw_addr + p * 64 + 16);
+            const f2 dx = f2_sub(f2_pack(P0.x, P0.y), jx), dy = f2_sub(f2_pack(P0.z, P0.w), jy),
+                     dz = f2_sub(f2_pack(P1.x, P1.y), jz);
+            r2v[p] = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+            float r2a, r2b;
+            f2_unpack(r2v[p], r2a, r2b);
+            anyp[p] = __any_sync(0xffffffffu, fminf(r2a, r2b) < a.rc2);
+        }
+        if (!(anyp[0] || anyp[1] || anyp[2] || anyp[3])) return;
+        f2 nx = 0ull, ny = 0ull, nz = 0ull; // jn: minus the j-side sums
+        float u_lj = 0.f, u_c = 0.f;
+
+        auto heavy = [&](const int p, const bool masked, const unsigned lm) {
+            const float4 P0 = mop_lds_v4(sw_addr + p * 64), P1 = mop_lds_v4(sw_addr + p * 64 + 16);
+            const f2 dx = f2_sub(f2_pack(P0.x, P0.y), jx), dy = f2_sub(f2_pack(P0.z, P0.w), jy),
+                     dz = f2_sub(f2_pack(P1.x, P1.y), jz), Qi = f2_pack(P1.z, P1.w);
+            float r2a, r2b;
+            f2_unpack(r2v[p], r2a, r2b);
+            bool ina = r2a < a.rc2, inb = r2b < a.rc2; // G8
+            if (masked) {
+                ina = ina && ((lm >> (2 * p)) & 1u);
+                inb = inb && ((lm >> (2 * p + 1)) & 1u);
+            }
+            float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
+            if (ENERGY) { // one Newton step: removes the approximation's bias from the energy sum
+                const float ea = __fmaf_rn(-__fmul_rn(r2a, ra), ra, 1.0f), eb = __fmaf_rn(-__fmul_rn(r2b, rb), rb, 1.0f);
+                ra = __fmaf_rn(0.5f * ra, ea, ra), rb = __fmaf_rn(0.5f * rb, eb, rb);
+            }
+            f2 S0 = 0ull, S1 = 0ull, S2 = 0ull;
+            unsigned ta, tb;
+            if (HVP) {
+                const float4 E0 = mop_lds_v4(sw_addr + p * 64 + 32), E1 = mop_lds_v4(sw_addr + p * 64 + 48);
+                S0 = f2_pack(E0.x, E0.y), S1 = f2_pack(E0.z, E0.w), S2 = f2_pack(E1.x, E1.y);
+                ta = (unsigned)__float_as_int(E1.z) + tj4, tb = (unsigned)__float_as_int(E1.w) + tj4;
+            } else {
+                const float2 T = mop_lds_v2(sw_addr + p * 64 + 56);
+                ta = (unsigned)__float_as_int(T.x) + tj4, tb = (unsigned)__float_as_int(T.y) + tj4;
+            }
+            const f2 c6 = f2_pack(mop_lds_f(ta), mop_lds_f(tb));
+            const f2 c12 = f2_pack(mop_lds_f(ta + off12), mop_lds_f(tb + off12));
+            const f2 rinv = f2_pack(ra, rb);
+            const f2 x = f2_mul(rinv, rinv);
+            const f2 x3 = f2_mul(f2_mul(x, x), x);
+            const f2 A = f2_mul(c6, x3);
+            const f2 B = f2_mul(f2_mul(c12, x3), x3);
+            const f2 qq = f2_mul(Qi, jq);
+            const f2 C = f2_mul(qq, f2_mul(x, rinv));
+            f2 gn = f2_fma(x, f2_sub(B, A), f2_fma(qq, nk2rf, C));
+            {
+                float ga, gb;
+                f2_unpack(gn, ga, gb);
+                gn = f2_pack(ina ? ga : 0.f, inb ? gb : 0.f);
+            }
+            if (!HVP) {
+                f2_acc(ax[p], gn, dx), f2_acc(ay[p], gn, dy), f2_acc(az[p], gn, dz);
+                f2_acc(nx, gn, dx), f2_acc(ny, gn, dy), f2_acc(nz, gn, dz);
+                if (ENERGY) {
+                    float x3a, x3b, qa, qb;
+                    f2_unpack(x3, x3a, x3b);
+                    f2_unpack(qq, qa, qb);
+                    const int ia = (int)((ta - tab6) >> 2), ib = (int)((tb - tab6) >> 2);
+                    const float2 ca = tabe[ia], cb = tabe[ib];
+                    const float ulja = __fmaf_rn(ca.y * x3a, x3a, -__fmaf_rn(ca.x, x3a, tabs[ia]));
+                    const float uljb = __fmaf_rn(cb.y * x3b, x3b, -__fmaf_rn(cb.x, x3b, tabs[ib]));
+                    const float uca = qa * (ra + a.krf * r2a - a.crf), ucb = qb * (rb + a.krf * r2b - a.crf);
+                    u_lj += (ina ? ulja : 0.f) + (inb ? uljb : 0.f);
+                    u_c += (ina ? uca : 0.f) + (inb ? ucb : 0.f);
+                }
+            } else {
+                f2 hn = f2_mul(x, f2_fma(C, f2_bc(-3.0f), f2_mul(x, f2_fma(B, f2_bc(-14.0f), f2_mul(A, f2_bc(8.0f))))));
+                {
+                    float ha, hb;
+                    f2_unpack(hn, ha, hb);
+                    hn = f2_pack(ina ? ha : 0.f, inb ? hb : 0.f);
+                }
+                const f2 ex = f2_sub(f2_bc(ce.x), S0), ey = f2_sub(f2_bc(ce.y), S1), ez = f2_sub(f2_bc(ce.z), S2);
+                const f2 tt = f2_mul(hn, f2_fma(dz, ez, f2_fma(dy, ey, f2_mul(dx, ex))));
+                f2_acc(ax[p], gn, ex), f2_acc(ay[p], gn, ey), f2_acc(az[p], gn, ez);
+                f2_acc(nx, gn, ex), f2_acc(ny, gn, ey), f2_acc(nz, gn, ez);
+                f2_acc(ax[p], tt, dx), f2_acc(ay[p], tt, dy), f2_acc(az[p], tt, dz);
+                f2_acc(nx, tt, dx), f2_acc(ny, tt, dy), f2_acc(nz, tt, dz);
+            }
+        };
+
+        const unsigned row1 = cur.y >> 8;
+        if (row1 == 0) { // no exclusions in this cluster pair
+#pragma unroll
+            for (int p = 0; p < 4; p++)
+                if (anyp[p]) heavy(p, false, 0u);
+        } else { // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
+            const uint4 *__restrict__ mrow =
+                reinterpret_cast<const uint4 *>(a.masks + (size_t)(un.excl_base + row1 - 1) * MOP_CI);
+            const uint4 m0 = mrow[0], m1 = mrow[1];
+            const unsigned mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+            unsigned lm = 0;
+#pragma unroll
+            for (int k = 0; k < MOP_CI; k++) lm |= ((mm[k] >> lane) & 1u) << k;
+#pragma unroll
+            for (int p = 0; p < 4; p++)
+                if (anyp[p]) heavy(p, true, lm);
+        }
+        {
+            float lx, hx, ly, hy, lz, hz;
+            f2_unpack(nx, lx, hx), f2_unpack(ny, ly, hy), f2_unpack(nz, lz, hz);
+            mop_red_add_f4(out + (cur.x * MOP_CJ + lane), -lx - hx, -ly - hy, -lz - hz);
+        }
+        if (ENERGY) e_lj += (double)u_lj, e_c += (double)u_c;
+    };
+
+    // ---- the unit's entries, 32 at a time: the chunk's entry words go to shared memory (one coalesced load), the
+    // j atoms of the next NBP_NST-1 entries are in flight (cp.async into the warp's ring; every lane copies and
+    // later reads only its own atom, so no cross-lane synchronisation is needed)
+    const unsigned eend = un.start + un.count;
+    for (unsigned c0 = un.start; c0 < eend; c0 += 32) {
+        const int nE = (int)min(32u, eend - c0);
+        __syncwarp();
+        if (lane < nE) {
+            const uint2 w = a.entries[c0 + lane];
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(se_addr + lane * 8), "r"(w.x), "r"(w.y) : "memory");
+        }
+        __syncwarp();
+        auto issue = [&](const int k) { // start the copies of entry k's j atoms into stage k % NBP_NST
+            if (k < nE) {
+                const unsigned jc = mop_lds_vu(se_addr + k * 8);
+                const unsigned o = jc * MOP_CJ + lane;
+                const unsigned st = sr_addr + (unsigned)(k % NBP_NST) * 1024u;
+                mop_cp_async16(st + lane16, xq + o);
+                if (HVP) mop_cp_async16(st + 512u + lane16, et + o);
+                else mop_cp_async4(st + 512u + lane * 4, typ + o);
+            }
+            mop_cp_commit();
+        };
+#pragma unroll
+        for (int k = 0; k < NBP_NST - 1; k++) issue(k);
+        for (int i = 0; i < nE; i++) {
+            issue(i + NBP_NST - 1);
+            mop_cp_wait<NBP_NST - 1>();
+            const unsigned st = sr_addr + (unsigned)(i % NBP_NST) * 1024u;
+            const uint2 cur = mop_lds_vu2(se_addr + i * 8);
+            const float4 cp = mop_lds_v4(st + lane16);
+            float4 ce = make_float4(0.f, 0.f, 0.f, 0.f);
+            unsigned tj4;
+            if (HVP) {
+                ce = mop_lds_v4(st + 512u + lane16);
+                tj4 = (unsigned)__float_as_int(ce.w) * 4u;
+            } else {
+                tj4 = mop_lds_vu(st + 512u + lane * 4) * 4u;
+            }
+            entry(cur, cp, ce, tj4);
+        }
+        mop_cp_wait<0>();
+    }
+
+    // ---- i side: 24 per-lane partial sums (8 atoms x 3 components) -> atom k = lane / 4.  Three halving
+    // exchanges (each lane keeps the half of the values its lane bits select) and two plain butterfly steps.
+    float v[24];
+#pragma unroll
+    for (int p = 0; p < 4; p++) {
+        f2_unpack(ax[p], v[6 * p + 0], v[6 * p + 3]);
+        f2_unpack(ay[p], v[6 * p + 1], v[6 * p + 4]);
+        f2_unpack(az[p], v[6 * p + 2], v[6 * p + 5]);
+    }
+#pragma unroll
+    for (int h = 12, bit = 16; h >= 3; h >>= 1, bit >>= 1) {
+        const bool up = (lane & bit) != 0;
+#pragma unroll
+        for (int j = 0; j < h; j++) {
+            const float keep = up ? v[j + h] : v[j], send = up ? v[j] : v[j + h];
+            v[j] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+        v[j] += __shfl_xor_sync(0xffffffffu, v[j], 2);
+        v[j] += __shfl_xor_sync(0xffffffffu, v[j], 1);
+    }
+    if ((lane & 3) == 0) mop_red_add_f4(out + (un.ci * MOP_CI + (lane >> 2)), v[0], v[1], v[2]);
+    if (ENERGY) {
+        e_lj = mop_warp_sum_d(e_lj), e_c = mop_warp_sum_d(e_c);
+        if (lane == 0) {
+            atomicAdd(&a.energies[0], e_lj);
+            atomicAdd(&a.energies[1], e_c);
+        }
+    }
+}
+
+template <int MODE, int VAR>
+__global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ? 5 : 4) k_nonbonded_p(const NbArgs a) {
+    extern __shared__ float4 s_dyn[];
+    char *sb = reinterpret_cast<char *>(s_dyn);
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float *sw = reinterpret_cast<float *>(sb) + w * 64;
+    const int n2 = a.nt * a.nt;
+    float *t6 = reinterpret_cast<float *>(sb + NBP_SM_TAB), *t12 = t6 + n2;
+    float2 *tabe = reinterpret_cast<float2 *>(t12 + n2);
+    float *tabs = reinterpret_cast<float *>(tabe + n2);
+    for (int t = threadIdx.x; t < n2; t += blockDim.x) {
+        const float2 c = a.tab[t];
+        t6[t] = c.x, t12[t] = c.y;
+        tabe[t] = a.tabe[t];
+        tabs[t] = a.tabs[t];
+    }
+    __syncthreads();
+    unsigned ubeg = 0, uend = a.ctr->n_units;
+    if (a.range == 0) uend = a.ctr->n_units_bead0;
+    else if (a.range == 1) ubeg = a.ctr->n_units_bead0;
+    const unsigned s0 = (unsigned)__cvta_generic_to_shared(sb);
+    const unsigned sw_addr = s0 + w * 256u, se_addr = s0 + NBP_SM_ENT + w * 256u;
+    const unsigned sr_addr = s0 + NBP_SM_RING + w * (NBP_NST * 1024u);
+    const unsigned tab6 = s0 + NBP_SM_TAB;
+    for (;;) {
+        unsigned u = 0;
+        if (lane == 0) u = atomicAdd(a.work, 1u);
+        u = __shfl_sync(0xffffffffu, u, 0) + ubeg;
+        if (u >= uend) break;
+        const uint4 *up = reinterpret_cast<const uint4 *>(a.units + u);
+        const uint4 u0 = up[0], u1 = up[1];
+        MopUnit un;
+        un.bead = (int)u0.x, un.ci = (int)u0.y, un.shift = (int)u0.z, un.start = u0.w;
+        un.count = u1.x, un.excl_base = u1.y;
+        if (un.count == 0) continue;
+        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabe, tabs, lane);
+    }
+}

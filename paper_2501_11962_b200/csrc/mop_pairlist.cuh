@@ -15,7 +15,7 @@ struct PlArgs {
     float rl, rl2; // list radius, and its square inflated by 1e-4 (conservative against FP32 rounding)
     const int *perm, *slot_of;
     const float4 *xq, *jlo, *jhi, *ilo, *ihi;
-    const int *col_start;
+    const int *col_start, *cell_rel, *col_count;
     const int *excl_start, *excl_list; // may be NULL
     MopUnit *units;
     MopEntry *entries;
@@ -121,89 +121,143 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
     __syncwarp();
     const int exN = s_exN[w];
 
-    // ---- scan the neighbouring columns under every periodic shift
-    const int nx = g.dims[0], ny = g.dims[1];
+    // ---- phase 1: candidate j-clusters.  Each lane takes one neighbouring column (under its x,y periodic image)
+    // and one z image; the column's z bins (S0's thin cells) give the slot range that can hold atoms within
+    // r_list in z, hence a short run of j-clusters.  The runs of the 32 lanes are enumerated flat (prefix sum +
+    // binary search), so every lane tests one cluster bounding box per iteration.
+    const int nx = g.dims[0], ny = g.dims[1], nz = g.dims[2];
     const int cx = mop_cell1(blo.x, g.sc[0], nx), cy = mop_cell1(blo.y, g.sc[1], ny);
     const int mx = (int)floorf(a.rl / g.colw[0]) + 1, my = (int)floorf(a.rl / g.colw[1]) + 1;
-    const float marg = 1.0e-4f;
+    const int wy = 2 * my + 1, noff = (2 * mx + 1) * wy;
+    const float marg = 1.0e-4f, mz = 1.0e-3f;
+    const float zlo = blo.z - a.rl - mz, zhi = bhi.z + a.rl + mz;
+    const int *cell_rel = a.cell_rel + (size_t)n * g.ncell;
+    const int *col_count = a.col_count + (size_t)n * g.ncol;
     int nbuf = 0;
-    unsigned shift_seen = 0;
-    unsigned nslots = 0;
-    for (int ox = -mx; ox <= mx; ox++) {
-        int gx = cx + ox;
-        int kx = gx < 0 ? -1 : (gx >= nx ? 1 : 0);
-        int colx = gx - kx * nx;
-        if (colx < 0 || colx >= nx) continue;
-        float sx = (float)kx * g.box[0];
-        float clo = (float)colx * g.colw[0] + sx;
-        float dxg = mop_gap(blo.x, bhi.x, clo - marg * g.box[0], clo + g.colw[0] + marg * g.box[0]);
-        if (dxg * dxg >= a.rl2) continue;
-        for (int oy = -my; oy <= my; oy++) {
-            int gy = cy + oy;
-            int ky = gy < 0 ? -1 : (gy >= ny ? 1 : 0);
-            int coly = gy - ky * ny;
-            if (coly < 0 || coly >= ny) continue;
-            float sy = (float)ky * g.box[1];
-            float cylo = (float)coly * g.colw[1] + sy;
-            float dyg = mop_gap(blo.y, bhi.y, cylo - marg * g.box[1], cylo + g.colw[1] + marg * g.box[1]);
-            if (dxg * dxg + dyg * dyg >= a.rl2) continue;
-            int col = colx * ny + coly;
-            int s0 = col_start[col], s1 = col_start[col + 1];
-            int c0 = s0 >> 5, nc = (s1 - s0) >> 5;
-            if (c0 + nc <= J0) continue; // whole column precedes the own j-cluster
-            for (int kz = -1; kz <= 1; kz++) {
-                if (kz == 1 && !(bhi.z + a.rl > g.box[2])) continue;
-                if (kz == -1 && !(blo.z - a.rl < 0.0f)) continue;
-                float sz = (float)kz * g.box[2];
-                unsigned sid = (unsigned)((kx + 1) + 3 * (ky + 1) + 9 * (kz + 1));
-                for (int b = 0; b < nc; b += 32) {
-                    int cj = c0 + b + lane;
-                    bool ok = (b + lane < nc) && cj >= J0;
-                    unsigned imask = 0;
-                    if (ok) {
-                        float4 lo = jlo[cj], hi = jhi[cj];
-                        ok = __float_as_int(lo.w) > 0;
-                        lo.x += sx, hi.x += sx, lo.y += sy, hi.y += sy, lo.z += sz, hi.z += sz;
-                        float ex = mop_gap(blo.x, bhi.x, lo.x, hi.x), ey = mop_gap(blo.y, bhi.y, lo.y, hi.y),
-                              ez = mop_gap(blo.z, bhi.z, lo.z, hi.z);
-                        ok = ok && (ex * ex + ey * ey + ez * ez < a.rl2);
-                        if (ok) {
-#pragma unroll
-                            for (int k = 0; k < MOP_CI; k++) {
-                                float4 p = ia[k];
-                                float px = mop_gap(p.x, p.x, lo.x, hi.x), py = mop_gap(p.y, p.y, lo.y, hi.y),
-                                      pz = mop_gap(p.z, p.z, lo.z, hi.z);
-                                if (p.w != 0.0f && px * px + py * py + pz * pz < a.rl2) imask |= 1u << k;
-                            }
-                            ok = imask != 0;
+    for (int kz = -1; kz <= 1; kz++) {
+        if (kz == -1 && !(zlo < 0.0f)) continue;
+        if (kz == 1 && !(zhi > g.box[2])) continue;
+        const float za = kz == 0 ? fmaxf(zlo, 0.0f) : (kz == -1 ? zlo + g.box[2] : 0.0f);
+        const float zb = kz == 0 ? fminf(zhi, g.box[2]) : (kz == -1 ? g.box[2] : zhi - g.box[2]);
+        const int b0 = max(mop_cell1(fmaxf(za, 0.0f), g.sc[2], nz) - 1, 0);
+        const int b1 = min(mop_cell1(fminf(zb, g.box[2]), g.sc[2], nz) + 1, nz - 1);
+        for (int ob = 0; ob < noff; ob += 32) {
+            const int t = ob + lane;
+            int first = 0, cnt = 0;
+            unsigned sid = 0;
+            if (t < noff) {
+                const int gx = cx + t / wy - mx, gy = cy + t % wy - my;
+                const int kx = gx < 0 ? -1 : (gx >= nx ? 1 : 0), ky = gy < 0 ? -1 : (gy >= ny ? 1 : 0);
+                const int colx = gx - kx * nx, coly = gy - ky * ny;
+                if (colx >= 0 && colx < nx && coly >= 0 && coly < ny) {
+                    const float clo = (float)colx * g.colw[0] + (float)kx * g.box[0];
+                    const float cylo = (float)coly * g.colw[1] + (float)ky * g.box[1];
+                    const float dxg = mop_gap(blo.x, bhi.x, clo - marg * g.box[0], clo + g.colw[0] + marg * g.box[0]);
+                    const float dyg = mop_gap(blo.y, bhi.y, cylo - marg * g.box[1], cylo + g.colw[1] + marg * g.box[1]);
+                    if (dxg * dxg + dyg * dyg < a.rl2) {
+                        const int col = colx * ny + coly;
+                        const int s0 = col_start[col];
+                        const int r0 = cell_rel[(size_t)col * nz + b0];
+                        const int r1 = b1 + 1 < nz ? cell_rel[(size_t)col * nz + b1 + 1] : col_count[col];
+                        if (r1 > r0) {
+                            first = max((s0 + r0) >> 5, J0); // half list: never below the own j-cluster
+                            cnt = max(((s0 + r1 - 1) >> 5) - first + 1, 0);
+                            sid = (unsigned)((kx + 1) + 3 * (ky + 1) + 9 * (kz + 1));
                         }
                     }
-                    unsigned row1 = 0;
-                    if (ok) {
-                        for (int t = 0; t < exN; t++)
-                            if (exJ[t] == cj) row1 = (unsigned)t + 1;
-                    }
-                    unsigned bal = __ballot_sync(0xffffffffu, ok);
-                    if (ok) {
-                        int pos = nbuf + __popc(bal & ((1u << lane) - 1));
-                        if (pos < MOP_LBUF) {
-                            bcj[pos] = cj;
-                            binfo[pos] = imask | (row1 << 8) | (sid << 16);
-                        }
-                        nslots += __popc(imask);
-                    }
-                    if (bal) shift_seen |= 1u << sid;
-                    nbuf += __popc(bal);
                 }
+            }
+            int incl = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            for (int base = 0; base < total; base += 32) {
+                const int f = base + lane;
+                int lo_s = 0, hi_s = 31;
+#pragma unroll
+                for (int it = 0; it < 5; it++) { // smallest lane s with incl[s] > f
+                    const int mid = (lo_s + hi_s) >> 1;
+                    const int v = __shfl_sync(0xffffffffu, incl, mid);
+                    if (v > f) hi_s = mid;
+                    else lo_s = mid + 1;
+                }
+                const int seg = min(lo_s, 31);
+                const int s_incl = __shfl_sync(0xffffffffu, incl, seg), s_cnt = __shfl_sync(0xffffffffu, cnt, seg);
+                const int s_first = __shfl_sync(0xffffffffu, first, seg);
+                const unsigned s_sid = __shfl_sync(0xffffffffu, sid, seg);
+                bool ok = f < total;
+                const int cj = s_first + (f - (s_incl - s_cnt));
+                if (ok) {
+                    float4 lo = jlo[cj], hi = jhi[cj];
+                    ok = __float_as_int(lo.w) > 0;
+                    float sx, sy, sz;
+                    mop_unit_shift((int)s_sid, g.box, sx, sy, sz);
+                    lo.x += sx, hi.x += sx, lo.y += sy, hi.y += sy, lo.z += sz, hi.z += sz;
+                    const float ex = mop_gap(blo.x, bhi.x, lo.x, hi.x), ey = mop_gap(blo.y, bhi.y, lo.y, hi.y),
+                                ez = mop_gap(blo.z, bhi.z, lo.z, hi.z);
+                    ok = ok && (ex * ex + ey * ey + ez * ez < a.rl2);
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    const int pos = nbuf + __popc(bal & ((1u << lane) - 1));
+                    if (pos < MOP_LBUF) {
+                        bcj[pos] = cj;
+                        binfo[pos] = s_sid;
+                    }
+                }
+                nbuf += __popc(bal);
             }
         }
     }
     __syncwarp();
-    if (nbuf == 0) return;
     if (nbuf > MOP_LBUF) {
         if (lane == 0) atomicOr(&a.ctr->overflow, 8u);
         nbuf = MOP_LBUF;
     }
+    // ---- phase 2: per candidate, which i atoms come within r_list of the j box (imask), and the exclusion row
+    unsigned shift_seen = 0;
+    unsigned nslots = 0;
+    for (int b = 0; b < nbuf; b += 32) {
+        const int idx = b + lane;
+        unsigned info = 0xffffffffu; // dead
+        if (idx < nbuf) {
+            const int cj = bcj[idx];
+            const unsigned sid = binfo[idx];
+            float4 lo = jlo[cj], hi = jhi[cj];
+            float sx, sy, sz;
+            mop_unit_shift((int)sid, g.box, sx, sy, sz);
+            lo.x += sx, hi.x += sx, lo.y += sy, hi.y += sy, lo.z += sz, hi.z += sz;
+            unsigned imask = 0;
+#pragma unroll
+            for (int k = 0; k < MOP_CI; k++) {
+                const float4 p = ia[k];
+                const float px = mop_gap(p.x, p.x, lo.x, hi.x), py = mop_gap(p.y, p.y, lo.y, hi.y),
+                            pz = mop_gap(p.z, p.z, lo.z, hi.z);
+                if (p.w != 0.0f && px * px + py * py + pz * pz < a.rl2) imask |= 1u << k;
+            }
+            if (imask != 0) {
+                unsigned row1 = 0;
+                for (int t = 0; t < exN; t++)
+                    if (exJ[t] == cj) row1 = (unsigned)t + 1;
+                info = imask | (row1 << 8) | (sid << 16);
+                nslots += __popc(imask);
+            }
+            binfo[idx] = info;
+        }
+        // the shifts that occur among the live candidates of this batch
+        unsigned live = __ballot_sync(0xffffffffu, info != 0xffffffffu);
+        while (live) {
+            const int l = __ffs(live) - 1;
+            const unsigned sidl = __shfl_sync(0xffffffffu, info, l) >> 16;
+            shift_seen |= 1u << sidl;
+            live &= ~__ballot_sync(0xffffffffu, info != 0xffffffffu && (info >> 16) == sidl);
+        }
+    }
+    __syncwarp();
+    if (shift_seen == 0) return;
     nslots = (unsigned)__reduce_add_sync(0xffffffffu, nslots);
     if (lane == 0) atomicAdd(a.slots_active, (unsigned long long)nslots);
 
@@ -224,7 +278,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         unsigned cnt = 0;
         for (int b = 0; b < nbuf; b += 32) {
             int idx = b + lane;
-            bool m = idx < nbuf && (binfo[idx] >> 16) == sid;
+            bool m = idx < nbuf && binfo[idx] != 0xffffffffu && (binfo[idx] >> 16) == sid;
             cnt += __popc(__ballot_sync(0xffffffffu, m));
         }
         if (cnt == 0) continue;
@@ -246,7 +300,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         unsigned wr = 0;
         for (int b = 0; b < nbuf; b += 32) {
             int idx = b + lane;
-            bool m = idx < nbuf && (binfo[idx] >> 16) == sid;
+            bool m = idx < nbuf && binfo[idx] != 0xffffffffu && (binfo[idx] >> 16) == sid;
             unsigned bal = __ballot_sync(0xffffffffu, m);
             if (m) {
                 unsigned pos = st + wr + __popc(bal & ((1u << lane) - 1));

@@ -34,7 +34,7 @@ UNIT = "bead-evals/s"
 FLOP_PER_PAIR_FORCE = 31.0
 FLOP_PER_PAIR_HVP = 55.0
 # DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None.
-TRAFFIC_BYTES_PER_LAUNCH = None
+TRAFFIC_BYTES_PER_LAUNCH = 130.6e6   # profiles/r01_ncu_summary.md: dram read 119.9 MB + write 10.7 MB (cfg 4, N = 8)
 
 
 def env_rank():
@@ -73,52 +73,86 @@ def throughput(units_total, ms_max):
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    """SM clock, power and throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe).  NVML is
+    polled from a thread every few ms (the timed region of the default run lasts ~0.1 s, shorter than one
+    nvidia-smi -lms period); nvidia-smi is the fallback when the NVML binding is missing."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index):
-        self.rows, self.proc, self.thread = [], None, None
+        self.rows, self.proc, self.thread, self.nvml, self.stop_flag = [], None, None, None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            idx = str(index)
+            self.h = (pynvml.nvmlDeviceGetHandleByUUID(idx) if idx.startswith("GPU-")
+                      else pynvml.nvmlDeviceGetHandleByIndex(int(idx)))
+            self.nvml = pynvml
+            self.smax = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                          "--format=csv,noheader,nounits", "-lms", "20"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
             self.proc = None
 
+    def _poll(self):
+        nv = self.nvml
+        bits = [(getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8), "hw_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40), "hw_thermal_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20), "sw_thermal_slowdown"),
+                (getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4), "sw_power_cap")]
+        while not self.stop_flag:
+            try:
+                sm = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.rows.append((time.perf_counter(), sm, self.smax, pw, [n for b, n in bits if r & b]))
+            except Exception:
+                pass
+            time.sleep(0.003)
+
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append((time.perf_counter(), line.strip()))
-
-    def stop(self, t0=None, t1=None):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "nvidia-smi unavailable"}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        sm, smax, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ts, line in self.rows:
-            if t0 is not None and not (t0 <= ts <= t1 + 0.2):
-                continue
-            f = [x.strip() for x in line.split(",")]
+            f = [x.strip() for x in line.strip().split(",")]
             if len(f) < 7:
                 continue
             try:
-                sm.append(float(f[0])), smax.append(float(f[1])), pw.append(float(f[2]))
+                self.rows.append((time.perf_counter(), float(f[0]), float(f[1]), float(f[2]),
+                                  [n for n, v in zip(self.NAMES, f[3:7]) if v.lower().startswith("active")]))
             except ValueError:
                 continue
-            for nme, v in zip(names, f[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nme)
-        if not sm:
+
+    def stop(self, t0=None, t1=None):
+        if self.nvml is None and self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "neither NVML nor nvidia-smi available"}
+        self.stop_flag = True
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+        elif self.thread is not None:
+            self.thread.join(timeout=1)
+        rows = [r for r in self.rows if t0 is None or t0 <= r[0] <= t1]
+        if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "no sample fell inside the timed region"}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(pw)),
-                "samples": len(sm), "reasons": sorted(reasons)}
+        reasons = sorted({n for r in rows for n in r[4]})
+        return {"sm_mhz": float(np.median([r[1] for r in rows])), "sm_max_mhz": float(max(r[2] for r in rows)),
+                "power_w_max": float(max(r[3] for r in rows)), "samples": len(rows), "reasons": reasons,
+                "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
 # ------------------------------------------------------------------------------------------------ workload
@@ -239,6 +273,7 @@ def run_ours(a):
     ach = pairs_hvp * FLOP_PER_PAIR_HVP / t_hvp / 1e12 if t_hvp > 0 else 0.0
     ach_f = pairs_force * FLOP_PER_PAIR_FORCE / t_force / 1e12 if t_force > 0 else 0.0
     ms_per_step = ms_max / a.steps
+    probe = binding.mop_probe_fp32(local_rank)   # FP32 pipe with and without register-file-limited operands
     out = {
         "metric": METRIC, "value": throughput(units, ms_max), "unit": UNIT, "n_gpus": world, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -256,6 +291,8 @@ def run_ours(a):
                      "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json); "
                                     "no measured FP32 entry exists" % (sm_max, peak_src),
                      "flop_per_pair": FLOP_PER_PAIR_HVP, "pairs_per_launch": pairs_hvp, "ms_per_launch": stages["S5_nb_hvp"],
+                     "fp32_probe_tflops": {k: round(v, 2) for k, v in probe.items() if k != "sms"},
+                     "frac_of_3reg_ffma2_probe": ach / probe["ffma2_3reg_tflops"] if probe["ffma2_3reg_tflops"] > 0 else None,
                      "force_kernel": {"achieved": ach_f, "frac": ach_f / peak_tf, "flop_per_pair": FLOP_PER_PAIR_FORCE,
                                       "pairs_per_launch": pairs_force, "ms_per_launch": stages["S2_nb_force"]}},
         "e2e": {"value": throughput(e2e_units, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": int(N) * Q * 12,

@@ -160,6 +160,14 @@ mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long long cap, long
  * This is the pass-2 kernel with eta := s.  Asynchronous. */
 mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float *s_dev, float *F_dev, float *Hs_dev);
 
+/* Measurement aid, not part of the path: achieved FP32 rate (TFLOP/s, FMA = 2 flop) of dependent-free FMA streams
+ * on all SMs of `device`, timed with CUDA events on the default stream (synchronises):
+ *   out[0] scalar FFMA with a reused operand (the nominal 128 lanes/clk/SM peak of DESIGN.md section 5),
+ *   out[1] scalar FFMA with three distinct register operands, out[2] packed FFMA2 (fma.rn.f32x2) with three
+ *   distinct register pairs -- the operand shape of the pair kernels' FMAs; out[3] = number of SMs.
+ * bench.py reports them beside the roofline.  Errors: INVALID_ARG (NULL), CUDA (no such device), OOM. */
+mop_status mop_probe_fp32(int device, double out[4]);
+
 #ifdef __cplusplus
 }
 #endif

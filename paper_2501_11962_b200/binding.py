@@ -17,7 +17,7 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
           4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
-           "mop_set_timing", "mop_get_timing"]
+           "mop_set_timing", "mop_get_timing", "mop_probe_fp32"]
 
 
 class MopError(RuntimeError):
@@ -72,11 +72,23 @@ def load(build_if_missing=True):
     L.mop_eval_veff_grad_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
     L.mop_set_timing.argtypes = [C.c_void_p, C.c_int]
     L.mop_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+    L.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    L.mop_probe_fp32.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
         getattr(L, n).restype = C.c_int
     _lib = L
     return L
+
+
+def mop_probe_fp32(device=0):
+    """Achieved TFLOP/s of dependent-free FMA streams (measurement aid, include/mop.h): reused-operand FFMA,
+    three-register FFMA, three-register-pair FFMA2."""
+    out = (C.c_double * 4)()
+    st = load().mop_probe_fp32(int(device), out)
+    if st != 0:
+        raise MopError(st, "mop_probe_fp32 failed")
+    return {"ffma_reuse_tflops": out[0], "ffma_3reg_tflops": out[1], "ffma2_3reg_tflops": out[2], "sms": int(out[3])}
 
 
 def _ptr(t):

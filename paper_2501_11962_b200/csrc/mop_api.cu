@@ -16,6 +16,7 @@
 #include "mop_nonbonded_packed.cuh"
 #include "mop_pairlist.cuh"
 #include "mop_path.cuh"
+#include "mop_probe.cuh"
 
 static thread_local char g_create_error[256] = "";
 
@@ -61,7 +62,7 @@ struct mop_ctx {
     float *d_G = 0;     // [N][Q][3] gradient for mop_step
     float *d_dbg = 0;   // [nf][Q][3]
     int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
-    int var_f = 8, var_h = 8;   // tuning variants of the pair kernels (NBV_* flags)
+    int var_f = 3, var_h = 3;   // tuning variants of the pair kernels (NBP_* flags: ILP2 | OCC5)
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
@@ -112,23 +113,16 @@ static cudaError_t dalloc(T **p, size_t n) {
 static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 typedef void (*nb_kernel_t)(const NbArgs);
-#define NB_VARIANTS(MODE)                                                                                         \
-    {k_nonbonded<MODE, 0>, k_nonbonded<MODE, 1>, k_nonbonded<MODE, 2>, k_nonbonded<MODE, 3>, k_nonbonded<MODE, 4>, \
-     k_nonbonded<MODE, 5>, k_nonbonded<MODE, 6>, k_nonbonded<MODE, 7>}
-static const nb_kernel_t k_force[8] = NB_VARIANTS(NB_FORCE);
-static const nb_kernel_t k_energy[8] = NB_VARIANTS(NB_ENERGY);
-static const nb_kernel_t k_hvp[8] = NB_VARIANTS(NB_HVP);
-// variants 8..15: the packed (f32x2) kernels, NBP_* flags in the low three bits
+// tuning variants of the pair kernels: NBP_* flags (mop_nonbonded_packed.cuh); MOP_NB_VAR / MOP_NB_VAR_H override
 #define NBP_VARIANTS(MODE)                                                                                    \
     {k_nonbonded_p<MODE, 0>, k_nonbonded_p<MODE, 1>, k_nonbonded_p<MODE, 2>, k_nonbonded_p<MODE, 3>,          \
      k_nonbonded_p<MODE, 4>, k_nonbonded_p<MODE, 5>, k_nonbonded_p<MODE, 6>, k_nonbonded_p<MODE, 7>}
 static const nb_kernel_t k_force_p[8] = NBP_VARIANTS(NB_FORCE);
 static const nb_kernel_t k_energy_p[8] = NBP_VARIANTS(NB_ENERGY);
 static const nb_kernel_t k_hvp_p[8] = NBP_VARIANTS(NB_HVP);
-static size_t nb_smem(const mop_ctx *c, int var) { return var >= 8 ? nbp_smem_bytes(c->nt) : nb_smem_bytes(c->nt); }
+static size_t nb_smem(const mop_ctx *c, int) { return nbp_smem_bytes(c->nt); }
 static nb_kernel_t nb_pick(int mode, int var) {
-    if (var >= 8) return (mode == NB_FORCE ? k_force_p : mode == NB_ENERGY ? k_energy_p : k_hvp_p)[var & 7];
-    return (mode == NB_FORCE ? k_force : mode == NB_ENERGY ? k_energy : k_hvp)[var & 7];
+    return (mode == NB_FORCE ? k_force_p : mode == NB_ENERGY ? k_energy_p : k_hvp_p)[var & 7];
 }
 
 extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_str() : g_create_error; }
@@ -412,8 +406,8 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     }
     // launch geometry of the persistent pair kernels
     {
-        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 15;
-        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 15;
+        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 7;
+        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 7;
         const void *fns[3] = {(const void *)nb_pick(NB_FORCE, c->var_f), (const void *)nb_pick(NB_ENERGY, c->var_f),
                               (const void *)nb_pick(NB_HVP, c->var_h)};
         int *nbs[3] = {&c->nb_blocks_f, &c->nb_blocks_fe, &c->nb_blocks_h};
@@ -770,4 +764,40 @@ extern "C" mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float 
     }
     CK(c, cudaGetLastError());
     return MOP_OK;
+}
+
+// FP32-pipe probe (measurement aid): TFLOP/s of dependent-free FMA streams, FMA = 2 flop
+extern "C" mop_status mop_probe_fp32(int device, double out[4]) {
+    if (!out) return MOP_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev || cudaSetDevice(device) != cudaSuccess) {
+        cudaGetLastError();
+        return MOP_ERR_CUDA;
+    }
+    int sms = 0;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    const int grid = sms * 4, block = 256;
+    float *buf = nullptr;
+    if (cudaMalloc((void **)&buf, (size_t)grid * block * sizeof(float)) != cudaSuccess) return MOP_ERR_OOM;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0), cudaEventCreate(&e1);
+    void (*ks[3])(float *, float) = {k_probe_fp32<0>, k_probe_fp32<1>, k_probe_fp32<2>};
+    const double fma_per_thread[3] = {8.0 * MOP_PROBE_ITER, 8.0 * MOP_PROBE_ITER, 16.0 * MOP_PROBE_ITER};
+    for (int m = 0; m < 3; m++) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; rep++) {
+            cudaEventRecord(e0);
+            ks[m]<<<grid, block>>>(buf, 1.0001f);
+            cudaEventRecord(e1);
+            cudaEventSynchronize(e1);
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        out[m] = 2.0 * fma_per_thread[m] * (double)grid * block / (best * 1e-3) / 1e12;
+    }
+    out[3] = (double)sms;
+    cudaEventDestroy(e0), cudaEventDestroy(e1);
+    cudaFree(buf);
+    return cudaGetLastError() == cudaSuccess ? MOP_OK : MOP_ERR_CUDA;
 }

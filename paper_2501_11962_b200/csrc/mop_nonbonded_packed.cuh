@@ -88,7 +88,8 @@ __device__ __forceinline__ void mop_cp_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
+enum { NBP_ILP2 = 1,    // fuse the pair math of two row pairs when both are needed (more ILP, more registers)
+       NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
        NBP_OCC6 = 4 };  // ask for 6 resident CTAs per SM (register cap 80)
 #define NBP_NST 4       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1)
 
@@ -231,18 +232,34 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 }
                 const f2 ex = f2_sub(f2_bc(ce.x), S0), ey = f2_sub(f2_bc(ce.y), S1), ez = f2_sub(f2_bc(ce.z), S2);
                 const f2 tt = f2_mul(hn, f2_fma(dz, ez, f2_fma(dy, ey, f2_mul(dx, ex))));
-                f2_acc(ax[p], gn, ex), f2_acc(ay[p], gn, ey), f2_acc(az[p], gn, ez);
-                f2_acc(nx, gn, ex), f2_acc(ny, gn, ey), f2_acc(nz, gn, ez);
-                f2_acc(ax[p], tt, dx), f2_acc(ay[p], tt, dy), f2_acc(az[p], tt, dz);
-                f2_acc(nx, tt, dx), f2_acc(ny, tt, dy), f2_acc(nz, tt, dz);
+                // v = tt d + gn e once, then two packed adds: fewer register-file reads than four FFMA2 per
+                // component (a three-register FFMA2 costs 3 issue cycles of the FP32 pipe, FMUL2/FADD2 cost 2)
+                const f2 vx = f2_fma(tt, dx, f2_mul(gn, ex)), vy = f2_fma(tt, dy, f2_mul(gn, ey)),
+                         vz = f2_fma(tt, dz, f2_mul(gn, ez));
+                ax[p] = f2_add(ax[p], vx), ay[p] = f2_add(ay[p], vy), az[p] = f2_add(az[p], vz);
+                nx = f2_add(nx, vx), ny = f2_add(ny, vy), nz = f2_add(nz, vz);
             }
         };
 
         const unsigned row1 = cur.y >> 8;
         if (row1 == 0) { // no exclusions in this cluster pair
+            if (VAR & NBP_ILP2) { // two row pairs in one basic block: two independent dependency chains per warp
 #pragma unroll
-            for (int p = 0; p < 4; p++)
-                if (anyp[p]) heavy(p, false, 0u);
+                for (int p = 0; p < 4; p += 2) {
+                    if (anyp[p] && anyp[p + 1]) {
+                        heavy(p, false, 0u);
+                        heavy(p + 1, false, 0u);
+                    } else if (anyp[p]) {
+                        heavy(p, false, 0u);
+                    } else if (anyp[p + 1]) {
+                        heavy(p + 1, false, 0u);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int p = 0; p < 4; p++)
+                    if (anyp[p]) heavy(p, false, 0u);
+            }
         } else { // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
             const uint4 *__restrict__ mrow =
                 reinterpret_cast<const uint4 *>(a.masks + (size_t)(un.excl_base + row1 - 1) * MOP_CI);

@@ -151,6 +151,34 @@ def test_config2_full_64_beads(B, oracle):
     m.close()
 
 
+def test_config4_full_size_bench_configuration(B, oracle):
+    """BASELINE.json configs[3] at full size (150,000 atoms, N = 8: the workload and launch configuration bench.py
+    times).  The path comes from the oracle's own force.  V_eff and the whole gradient against the oracle; the
+    in-range pair COUNT of every force bead, and the pair SET restricted to a sample of i atoms, bit-exact;
+    momentum conservation (P6) on the GPU's F and H.eta at this size."""
+    s = W.config4(seed=0, n_beads=8)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 8, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    m = B.Mop(s, 8)
+    v, g = m.mop_eval_veff_grad(R)
+    v_ref, g_ref, parts = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=False, want_parts=True)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    assert H.rms_rel(m.mop_debug_get("F"), parts["F"]) <= TOL_RMS
+    assert H.rms_rel(m.mop_debug_get("Heta"), parts["Heta"]) <= TOL_RMS
+    for arr in (m.mop_debug_get("F"), m.mop_debug_get("Heta")):
+        a = arr.astype(np.float64)
+        assert np.abs(a.sum(1)).max() <= 1e-4 * np.abs(a).sum(1).max()
+    ref = oracle.pairs(o, R[0].astype(np.float64), geom=1, brute=False)
+    got, cnt = m.mop_debug_pairs(0)
+    assert cnt == len(ref), "pair count differs on bead 0: %d vs %d" % (cnt, len(ref))
+    pick = lambda P: P[(P[:, 0] % 97 == 0) | (P[:, 1] % 97 == 0)]
+    assert np.array_equal(pick(got), pick(ref)), "sampled pair set differs on bead 0"
+    n_last = oracle.bead(o, R[m.nf - 1].astype(np.float64), geom=1, want_force=False)["npairs"]
+    assert m.mop_debug_pairs(m.nf - 1, cap=0)[1] == n_last
+    m.close()
+
+
 def test_async_eval_matches_sync_and_repeats(B, oracle):
     """veff_out = NULL leaves the value in the context; repeated evaluations agree to float-atomic noise."""
     s, o, R = case(oracle, "c2")

@@ -62,7 +62,7 @@ struct mop_ctx {
     float *d_G = 0;     // [N][Q][3] gradient for mop_step
     float *d_dbg = 0;   // [nf][Q][3]
     int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
-    int var_f = 3, var_h = 3;   // tuning variants of the pair kernels (NBP_* flags: ILP2 | OCC5)
+    int var_f = 2, var_h = 2;   // tuning variants of the pair kernels (NBP_* flags; 2 = five CTAs per SM)
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;

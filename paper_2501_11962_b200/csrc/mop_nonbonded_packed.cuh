@@ -88,8 +88,7 @@ __device__ __forceinline__ void mop_cp_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-enum { NBP_ILP2 = 1,    // fuse the pair math of two row pairs when both are needed (more ILP, more registers)
-       NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
+enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
        NBP_OCC6 = 4 };  // ask for 6 resident CTAs per SM (register cap 80)
 #define NBP_NST 4       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1)
 
@@ -98,18 +97,19 @@ enum { NBP_ILP2 = 1,    // fuse the pair math of two row pairs when both are nee
 //                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
 //   [1024, 2048)           the current chunk of up to 32 list entries, 256 B per warp
 //   [2048, 2048 + 16 KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
-//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), (C6, C12)[nt*nt] as given, energy shift [nt*nt]
+//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), (C6, C12)[nt*nt] as given, energy shift [nt*nt],
+//   and one flag per type: its LJ row has a non-zero entry
 #define NBP_SM_ENT 1024u
 #define NBP_SM_RING 2048u
 #define NBP_SM_TAB (2048u + 4u * NBP_NST * 1024u)
-__host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 20; }
+__host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 20 + (size_t)nt * 4; }
 
 template <int MODE, int VAR>
 __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, float *__restrict__ sw,
                                          const unsigned sw_addr, const unsigned se_addr, const unsigned sr_addr,
                                          const unsigned tab6, const unsigned off12,
                                          const float2 *__restrict__ tabe, const float *__restrict__ tabs,
-                                         const int lane) {
+                                         const int *__restrict__ tflag, const int lane) {
     constexpr bool HVP = MODE == NB_HVP, ENERGY = MODE == NB_ENERGY;
     const unsigned boff = (unsigned)un.bead * (unsigned)a.S; // nf * S < 2^31 (checked at create)
     const float4 *__restrict__ xq = a.xq + boff;
@@ -118,6 +118,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     float4 *__restrict__ out = a.out + boff;
 
     __syncwarp();
+    bool has_lj = false;
     if (lane < MOP_CI) {
         float sx, sy, sz;
         mop_unit_shift(un.shift, a.box, sx, sy, sz);
@@ -130,6 +131,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         } else {
             ti = typ[un.ci * MOP_CI + lane];
         }
+        has_lj = tflag[ti] != 0;
         float *d = sw + (lane >> 1) * 16 + (lane & 1);
         d[0] = __fsub_rn(p.x, sx), d[2] = __fsub_rn(p.y, sy), d[4] = __fsub_rn(p.z, sz);
         d[6] = p.w * MOP_KE;
@@ -137,6 +139,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         d[14] = __int_as_float((int)tab6 + ti * a.nt * 4);
     }
     __syncwarp();
+    const unsigned ljmask = __ballot_sync(0xffffffffu, has_lj) & 0xffu; // bit k: i atom k has a non-zero LJ row
 
     f2 ax[4], ay[4], az[4];
 #pragma unroll
@@ -167,7 +170,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         f2 nx = 0ull, ny = 0ull, nz = 0ull; // jn: minus the j-side sums
         float u_lj = 0.f, u_c = 0.f;
 
-        auto heavy = [&](const int p, const bool masked, const unsigned lm) {
+        auto heavy = [&](const int p, const bool masked, const unsigned lm, const bool nolj) {
             const float4 P0 = mop_lds_v4(sw_addr + p * 64), P1 = mop_lds_v4(sw_addr + p * 64 + 16);
             const f2 dx = f2_sub(f2_pack(P0.x, P0.y), jx), dy = f2_sub(f2_pack(P0.z, P0.w), jy),
                      dz = f2_sub(f2_pack(P1.x, P1.y), jz), Qi = f2_pack(P1.z, P1.w);
@@ -193,16 +196,21 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 const float2 T = mop_lds_v2(sw_addr + p * 64 + 56);
                 ta = (unsigned)__float_as_int(T.x) + tj4, tb = (unsigned)__float_as_int(T.y) + tj4;
             }
-            const f2 c6 = f2_pack(mop_lds_f(ta), mop_lds_f(tb));
-            const f2 c12 = f2_pack(mop_lds_f(ta + off12), mop_lds_f(tb + off12));
             const f2 rinv = f2_pack(ra, rb);
             const f2 x = f2_mul(rinv, rinv);
-            const f2 x3 = f2_mul(f2_mul(x, x), x);
-            const f2 A = f2_mul(c6, x3);
-            const f2 B = f2_mul(f2_mul(c12, x3), x3);
             const f2 qq = f2_mul(Qi, jq);
             const f2 C = f2_mul(qq, f2_mul(x, rinv));
-            f2 gn = f2_fma(x, f2_sub(B, A), f2_fma(qq, nk2rf, C));
+            f2 x3 = 0ull, A = 0ull, B = 0ull, gn;
+            if (nolj) { // both i atoms have an all-zero LJ row (water hydrogens): reaction field only
+                gn = f2_fma(qq, nk2rf, C);
+            } else {
+                const f2 c6 = f2_pack(mop_lds_f(ta), mop_lds_f(tb));
+                const f2 c12 = f2_pack(mop_lds_f(ta + off12), mop_lds_f(tb + off12));
+                x3 = f2_mul(f2_mul(x, x), x);
+                A = f2_mul(c6, x3);
+                B = f2_mul(f2_mul(c12, x3), x3);
+                gn = f2_fma(x, f2_sub(B, A), f2_fma(qq, nk2rf, C));
+            }
             {
                 float ga, gb;
                 f2_unpack(gn, ga, gb);
@@ -217,14 +225,15 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                     f2_unpack(qq, qa, qb);
                     const int ia = (int)((ta - tab6) >> 2), ib = (int)((tb - tab6) >> 2);
                     const float2 ca = tabe[ia], cb = tabe[ib];
-                    const float ulja = __fmaf_rn(ca.y * x3a, x3a, -__fmaf_rn(ca.x, x3a, tabs[ia]));
-                    const float uljb = __fmaf_rn(cb.y * x3b, x3b, -__fmaf_rn(cb.x, x3b, tabs[ib]));
+                    const float ulja = nolj ? 0.f : __fmaf_rn(ca.y * x3a, x3a, -__fmaf_rn(ca.x, x3a, tabs[ia]));
+                    const float uljb = nolj ? 0.f : __fmaf_rn(cb.y * x3b, x3b, -__fmaf_rn(cb.x, x3b, tabs[ib]));
                     const float uca = qa * (ra + a.krf * r2a - a.crf), ucb = qb * (rb + a.krf * r2b - a.crf);
                     u_lj += (ina ? ulja : 0.f) + (inb ? uljb : 0.f);
                     u_c += (ina ? uca : 0.f) + (inb ? ucb : 0.f);
                 }
             } else {
-                f2 hn = f2_mul(x, f2_fma(C, f2_bc(-3.0f), f2_mul(x, f2_fma(B, f2_bc(-14.0f), f2_mul(A, f2_bc(8.0f))))));
+                f2 hn = nolj ? f2_mul(f2_mul(x, f2_bc(-3.0f)), C)
+                             : f2_mul(x, f2_fma(C, f2_bc(-3.0f), f2_mul(x, f2_fma(B, f2_bc(-14.0f), f2_mul(A, f2_bc(8.0f))))));
                 {
                     float ha, hb;
                     f2_unpack(hn, ha, hb);
@@ -243,23 +252,12 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
 
         const unsigned row1 = cur.y >> 8;
         if (row1 == 0) { // no exclusions in this cluster pair
-            if (VAR & NBP_ILP2) { // two row pairs in one basic block: two independent dependency chains per warp
 #pragma unroll
-                for (int p = 0; p < 4; p += 2) {
-                    if (anyp[p] && anyp[p + 1]) {
-                        heavy(p, false, 0u);
-                        heavy(p + 1, false, 0u);
-                    } else if (anyp[p]) {
-                        heavy(p, false, 0u);
-                    } else if (anyp[p + 1]) {
-                        heavy(p + 1, false, 0u);
-                    }
+            for (int p = 0; p < 4; p++)
+                if (anyp[p]) {
+                    if ((ljmask >> (2 * p)) & 3u) heavy(p, false, 0u, false);
+                    else heavy(p, false, 0u, true);
                 }
-            } else {
-#pragma unroll
-                for (int p = 0; p < 4; p++)
-                    if (anyp[p]) heavy(p, false, 0u);
-            }
         } else { // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
             const uint4 *__restrict__ mrow =
                 reinterpret_cast<const uint4 *>(a.masks + (size_t)(un.excl_base + row1 - 1) * MOP_CI);
@@ -270,7 +268,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             for (int k = 0; k < MOP_CI; k++) lm |= ((mm[k] >> lane) & 1u) << k;
 #pragma unroll
             for (int p = 0; p < 4; p++)
-                if (anyp[p]) heavy(p, true, lm);
+                if (anyp[p]) {
+                    if ((ljmask >> (2 * p)) & 3u) heavy(p, true, lm, false);
+                    else heavy(p, true, lm, true);
+                }
         }
         {
             float lx, hx, ly, hy, lz, hz;
@@ -367,11 +368,17 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
     float *t6 = reinterpret_cast<float *>(sb + NBP_SM_TAB), *t12 = t6 + n2;
     float2 *tabe = reinterpret_cast<float2 *>(t12 + n2);
     float *tabs = reinterpret_cast<float *>(tabe + n2);
+    int *tflag = reinterpret_cast<int *>(tabs + n2);   // [nt]: 1 iff the type's LJ row has a non-zero entry
     for (int t = threadIdx.x; t < n2; t += blockDim.x) {
         const float2 c = a.tab[t];
         t6[t] = c.x, t12[t] = c.y;
         tabe[t] = a.tabe[t];
         tabs[t] = a.tabs[t];
+    }
+    for (int t = threadIdx.x; t < a.nt; t += blockDim.x) {
+        int f = 0;
+        for (int u = 0; u < a.nt; u++) f |= (a.tab[t * a.nt + u].x != 0.f || a.tab[t * a.nt + u].y != 0.f);
+        tflag[t] = f;
     }
     __syncthreads();
     unsigned ubeg = 0, uend = a.ctr->n_units;
@@ -392,6 +399,6 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
         un.bead = (int)u0.x, un.ci = (int)u0.y, un.shift = (int)u0.z, un.start = u0.w;
         un.count = u1.x, un.excl_base = u1.y;
         if (un.count == 0) continue;
-        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabe, tabs, lane);
+        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabe, tabs, tflag, lane);
     }
 }

@@ -181,10 +181,11 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 ina = ina && ((lm >> (2 * p)) & 1u);
                 inb = inb && ((lm >> (2 * p + 1)) & 1u);
             }
-            float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
+            const float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
+            f2 rinv = f2_pack(ra, rb);
             if (ENERGY) { // one Newton step: removes the approximation's bias from the energy sum
-                const float ea = __fmaf_rn(-__fmul_rn(r2a, ra), ra, 1.0f), eb = __fmaf_rn(-__fmul_rn(r2b, rb), rb, 1.0f);
-                ra = __fmaf_rn(0.5f * ra, ea, ra), rb = __fmaf_rn(0.5f * rb, eb, rb);
+                const f2 em = f2_fma(f2_mul(r2v[p], rinv), rinv, f2_bc(-1.0f));   // r2 rinv^2 - 1
+                rinv = f2_fma(f2_mul(rinv, f2_bc(-0.5f)), em, rinv);
             }
             f2 S0 = 0ull, S1 = 0ull, S2 = 0ull;
             unsigned ta, tb;
@@ -196,7 +197,6 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 const float2 T = mop_lds_v2(sw_addr + p * 64 + 56);
                 ta = (unsigned)__float_as_int(T.x) + tj4, tb = (unsigned)__float_as_int(T.y) + tj4;
             }
-            const f2 rinv = f2_pack(ra, rb);
             const f2 x = f2_mul(rinv, rinv);
             const f2 qq = f2_mul(Qi, jq);
             const f2 C = f2_mul(qq, f2_mul(x, rinv));
@@ -219,17 +219,18 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             if (!HVP) {
                 f2_acc(ax[p], gn, dx), f2_acc(ay[p], gn, dy), f2_acc(az[p], gn, dz);
                 f2_acc(nx, gn, dx), f2_acc(ny, gn, dy), f2_acc(nz, gn, dz);
-                if (ENERGY) {
-                    float x3a, x3b, qa, qb;
-                    f2_unpack(x3, x3a, x3b);
-                    f2_unpack(qq, qa, qb);
-                    const int ia = (int)((ta - tab6) >> 2), ib = (int)((tb - tab6) >> 2);
-                    const float2 ca = tabe[ia], cb = tabe[ib];
-                    const float ulja = nolj ? 0.f : __fmaf_rn(ca.y * x3a, x3a, -__fmaf_rn(ca.x, x3a, tabs[ia]));
-                    const float uljb = nolj ? 0.f : __fmaf_rn(cb.y * x3b, x3b, -__fmaf_rn(cb.x, x3b, tabs[ib]));
-                    const float uca = qa * (ra + a.krf * r2a - a.crf), ucb = qb * (rb + a.krf * r2b - a.crf);
-                    u_lj += (ina ? ulja : 0.f) + (inb ? uljb : 0.f);
-                    u_c += (ina ? uca : 0.f) + (inb ? ucb : 0.f);
+                if (ENERGY) { // u_lj = C12 x^6 - C6 x^3 - shift = B/12 - A/6 - shift;  u_c = ke qi qj (1/r + k_rf r^2 - c_rf)
+                    f2 ue = f2_mul(qq, f2_add(f2_fma(r2v[p], f2_bc(a.krf), rinv), f2_bc(-a.crf)));
+                    if (!nolj) {
+                        const f2 sh = f2_pack(mop_lds_f(ta + 4u * off12), mop_lds_f(tb + 4u * off12));
+                        const f2 ul = f2_fma(B, f2_bc(1.0f / 12.0f), f2_fma(A, f2_bc(-1.0f / 6.0f), f2_mul(sh, f2_bc(-1.0f))));
+                        float la, lb;
+                        f2_unpack(ul, la, lb);
+                        u_lj += (ina ? la : 0.f) + (inb ? lb : 0.f);
+                    }
+                    float ca, cb;
+                    f2_unpack(ue, ca, cb);
+                    u_c += (ina ? ca : 0.f) + (inb ? cb : 0.f);
                 }
             } else {
                 f2 hn = nolj ? f2_mul(f2_mul(x, f2_bc(-3.0f)), C)

@@ -74,47 +74,49 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
     __syncwarp();
 
     // ---- exclusion rows: for each i atom, clear the bit of every excluded partner in its j-cluster's row
+    // (four lanes per i atom, so the dependent loads perm -> excl_start -> excl_list -> slot_of of the 8 atoms are
+    // in flight together instead of one atom after the other)
     if (a.excl_start != nullptr) {
-        for (int k = 0; k < MOP_CI; k++) {
-            int orig = perm[ci * MOP_CI + k];
-            if (orig < 0) continue;
-            int e0 = a.excl_start[orig], e1 = a.excl_start[orig + 1];
-            for (int eb = e0; eb < e1; eb += 32) {
-                int e = eb + lane;
-                bool act = e < e1;
-                int J = -1, bit = 0;
-                if (act) {
-                    int ps = slot_of[a.excl_list[e]];
-                    J = ps >> 5;
-                    bit = ps & 31;
-                    if (J < J0) act = false; // never listed from this side
-                }
-                unsigned pend = __ballot_sync(0xffffffffu, act);
-                while (pend) {
-                    int leader = __ffs(pend) - 1;
-                    int Jl = __shfl_sync(0xffffffffu, J, leader);
-                    int nrow = s_exN[w];
-                    unsigned hit = __ballot_sync(0xffffffffu, lane < nrow && exJ[lane] == Jl);
-                    int row;
-                    if (hit) {
-                        row = __ffs(hit) - 1;
-                    } else if (nrow < MOP_EXROWS) {
-                        row = nrow;
-                        if (lane == 0) {
-                            exJ[nrow] = Jl;
-                            s_exN[w] = nrow + 1;
-                        }
-                        if (lane < MOP_CI) exM[nrow][lane] = 0xffffffffu;
-                    } else {
-                        row = -1;
-                        if (lane == 0) atomicOr(&a.ctr->overflow, 16u);
+        const int k = lane >> 2, sub = lane & 3;
+        const int orig = perm[ci * MOP_CI + k];
+        int e0 = 0, e1 = 0;
+        if (orig >= 0) e0 = a.excl_start[orig], e1 = a.excl_start[orig + 1];
+        const int maxn = __reduce_max_sync(0xffffffffu, e1 - e0);
+        for (int eb = 0; eb < maxn; eb += 4) {
+            const int e = e0 + eb + sub;
+            bool act = e < e1;
+            int J = -1, bit = 0;
+            if (act) {
+                const int ps = slot_of[a.excl_list[e]];
+                J = ps >> 5;
+                bit = ps & 31;
+                if (J < J0) act = false; // never listed from this side
+            }
+            unsigned pend = __ballot_sync(0xffffffffu, act);
+            while (pend) {
+                const int leader = __ffs(pend) - 1;
+                const int Jl = __shfl_sync(0xffffffffu, J, leader);
+                const int nrow = s_exN[w];
+                const unsigned hit = __ballot_sync(0xffffffffu, lane < nrow && exJ[lane] == Jl);
+                int row;
+                if (hit) {
+                    row = __ffs(hit) - 1;
+                } else if (nrow < MOP_EXROWS) {
+                    row = nrow;
+                    if (lane == 0) {
+                        exJ[nrow] = Jl;
+                        s_exN[w] = nrow + 1;
                     }
-                    __syncwarp();
-                    bool same = act && J == Jl;
-                    if (same && row >= 0) atomicAnd(&exM[row][k], ~(1u << bit));
-                    pend &= ~__ballot_sync(0xffffffffu, same);
-                    __syncwarp();
+                    if (lane < MOP_CI) exM[nrow][lane] = 0xffffffffu;
+                } else {
+                    row = -1;
+                    if (lane == 0) atomicOr(&a.ctr->overflow, 16u);
                 }
+                __syncwarp();
+                const bool same = act && J == Jl;
+                if (same && row >= 0) atomicAnd(&exM[row][k], ~(1u << bit));
+                pend &= ~__ballot_sync(0xffffffffu, same);
+                __syncwarp();
             }
         }
     }

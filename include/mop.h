@@ -54,8 +54,10 @@ typedef struct {
     int n_beads;      /* N >= 1 */
     float box[3];     /* rectangular periodic box (nm) */
     float r_cut;      /* nonbonded cutoff (nm), > 0 */
-    float r_buf;      /* Verlet buffer (nm), >= 0.  0: the pair list is rebuilt in every evaluation.  > 0: the
-                         list (built with r_cut + r_buf) is reused until an atom has moved more than r_buf/2 */
+    float r_buf;      /* list margin (nm), >= 0: the cluster-pair list is built with r_cut + r_buf.  This build rebuilds
+                         the list in EVERY evaluation (bench.py times it that way), so 0 is the efficient value; reuse
+                         of a buffered list across evaluations is not implemented.  Results never depend on r_buf:
+                         the r_cut test is applied per atom pair in the pair kernels */
     float eps_rf;     /* reaction-field dielectric; <= 0 means infinity (k_rf = 1/(2 r_cut^3)) */
     int lj_shift;     /* 1: potential-shift the LJ energy so that U_LJ(r_cut) = 0 (forces unchanged) */
     double dt_path;   /* path spacing Delta t (ps): enters K_i and L^n only */

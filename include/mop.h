@@ -162,6 +162,17 @@ mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long long cap, long
  * This is the pass-2 kernel with eta := s.  Asynchronous. */
 mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float *s_dev, float *F_dev, float *Hs_dev);
 
+/* The same V_eff and gradient with the Hessian term of eqs (5),(6) evaluated the way the paper does it
+ * (PAPER.md:61-70, 107-110): the central finite difference [F(R^n + eps eta^n) - F(R^n - eps eta^n)] / (4 eps) of two
+ * displaced force evaluations (PMD kernels 2, 3) instead of the analytic -1/2 H^n eta^n.  eps > 0 is the paper's
+ * dimensionless epsilon, one value for all beads (PAPER.md:64 leaves it open: "small enough"; eps * max|eta| of 1e-5 to
+ * 1e-4 nm keeps both the truncation and the FP32 cancellation error small).  Costs three force passes per bead, each
+ * displaced configuration with its own cell list and pair list.  With a plain cutoff a pair that crosses r_cut between
+ * R + eps eta and R - eps eta contributes its force jump divided by 4 eps (reading G9); the analytic form has no such term.
+ * R_dev, grad_dev DEVICE [N][Q][3] (grad_dev required); veff_out HOST or NULL as in mop_eval_veff_grad.  After this
+ * call mop_debug_get / mop_debug_pairs describe the last displaced configuration.  Errors: INVALID_ARG, OOM, CUDA. */
+mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, double eps, double *veff_out, float *grad_dev);
+
 /* Measurement aid, not part of the path: achieved FP32 rate (TFLOP/s, FMA = 2 flop) of dependent-free FMA streams
  * on all SMs of `device`, timed with CUDA events on the default stream (synchronises):
  *   out[0] scalar FFMA with a reused operand (the nominal 128 lanes/clk/SM peak of DESIGN.md section 5),

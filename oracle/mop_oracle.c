@@ -21,6 +21,8 @@
  *                      L^n = dt/(m nu) F^n  (reading G1 in DESIGN.md: the
  *                      printed L^n is inverted; eqs (5)-(7) require K*L/F = 1/2)
  *   O5 grad V_eff      derivative of eq. (3); equals -(eqs 5,6,7)
+ *   O5-FD              the same gradient with the paper's own finite-difference
+ *                      Hessian term, eqs (5),(6),(7) as printed (orc_veff_grad_fd)
  *   O6 integrator      velocity Verlet on eq. (4)
  *
  * Geometry modes (argument `geom`):
@@ -667,6 +669,79 @@ double orc_veff_grad(const orc_system *s, int N, const double *R, int geom, int 
     free(U);
     free(np);
     free(X);
+    return veff;
+}
+
+/* ------------------------------------------------------------------ */
+/* O5-FD: the paper's effective force as printed, eqs (5),(6),(7)      */
+/* (PAPER.md:61-70), with the Hessian term as the finite difference     */
+/*   [F(R^n + eps eta^n) - F(R^n - eps eta^n)] / (4 eps),               */
+/*   eta^n = R^{n+1} - R^n - L^n  (L^n = a F^n, reading G1) */
+/* eps is the paper's dimensionless epsilon, the same for every bead.   */
+/* grad [N][Q][3] receives -F_eff^n; returns V_eff (eq. 3).             */
+/* In geom 1 the displaced coordinates are rounded to float like every  */
+/* other position (inside orc_bead) before wrap, predicate and physics. */
+/* ------------------------------------------------------------------ */
+double orc_veff_grad_fd(const orc_system *s, int N, const double *R, double eps, int geom, int brute, double *grad) {
+    int Q = s->n_atoms;
+    size_t bead = 3 * (size_t)Q;
+    int nf = (N > 1) ? N - 1 : 1;
+    double *F = (double *)malloc(sizeof(double) * bead * (size_t)nf);
+    double *Fp = (double *)calloc(bead * (size_t)nf, sizeof(double));
+    double *Fm = (double *)calloc(bead * (size_t)nf, sizeof(double));
+    double *Rp = (double *)malloc(sizeof(double) * bead * (size_t)nf);
+    double *Rm = (double *)malloc(sizeof(double) * bead * (size_t)nf);
+    double *U = (double *)calloc((size_t)nf * 4, sizeof(double));
+    double *X = (double *)malloc(sizeof(double) * bead * (size_t)N);
+    for (size_t i = 0; i < bead * (size_t)N; i++) X[i] = geom ? (double)(float)R[i] : R[i];
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int n = 0; n < nf; n++) orc_bead(s, R + bead * n, geom, brute, F + bead * n, NULL, NULL, U + 4 * n);
+    double e_spring = 0.0;
+    if (N > 1) {
+        for (int n = 0; n < N - 1; n++)
+            for (int i = 0; i < Q; i++) {
+                double m = (double)s->mass[i];
+                double a = s->dt_path / (m * s->nu);
+                double K = m * s->nu / (2.0 * s->dt_path);
+                for (int q = 0; q < 3; q++) {
+                    size_t o = bead * n + 3 * (size_t)i + q;
+                    double e = (X[o + bead] - X[o]) - a * F[o]; /* eta^n */
+                    e_spring += 0.5 * K * e * e;
+                    Rp[o] = X[o] + eps * e;                     /* paper kernel 2 */
+                    Rm[o] = X[o] - eps * e;
+                }
+            }
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int n = 0; n < 2 * (N - 1); n++) {
+            int b = n >> 1;
+            if (n & 1) orc_bead(s, Rm + bead * b, geom, brute, Fm + bead * b, NULL, NULL, NULL);
+            else orc_bead(s, Rp + bead * b, geom, brute, Fp + bead * b, NULL, NULL, NULL);
+        }
+    }
+    double veff = U[0] + U[1] + U[2] + U[3] + e_spring;
+    if (grad) {
+        for (int n = 0; n < N; n++)
+            for (int i = 0; i < Q; i++) {
+                double m = (double)s->mass[i];
+                double K = m * s->nu / (2.0 * s->dt_path);
+                for (int q = 0; q < 3; q++) {
+                    size_t o = bead * n + 3 * (size_t)i + q;
+                    double feff;
+                    if (N == 1) {
+                        feff = F[o];                                                   /* V_eff = U(R^1) */
+                    } else if (n == 0) {                                               /* eq. (6) */
+                        feff = 0.5 * F[o] + K * (X[o + bead] - X[o]) + (Fp[o] - Fm[o]) / (4.0 * eps);
+                    } else if (n < N - 1) {                                            /* eq. (5) */
+                        feff = -K * (2.0 * X[o] - X[o - bead] - X[o + bead]) + 0.5 * (F[o - bead] - F[o]) +
+                               (Fp[o] - Fm[o]) / (4.0 * eps);
+                    } else {                                                           /* eq. (7) */
+                        feff = -K * (X[o] - X[o - bead]) + 0.5 * F[o - bead];
+                    }
+                    grad[o] = -feff;
+                }
+            }
+    }
+    free(F), free(Fp), free(Fm), free(Rp), free(Rm), free(U), free(X);
     return veff;
 }
 

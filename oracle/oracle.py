@@ -52,6 +52,7 @@ def _load():
         L.orc_pairs.restype = C.c_long
         L.orc_bead.restype = C.c_long
         L.orc_veff_grad.restype = C.c_double
+        L.orc_veff_grad_fd.restype = C.c_double
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -196,6 +197,18 @@ def veff_grad(osys, R, geom=0, brute=False, want_parts=False):
     if want_parts:
         return float(v), grad, dict(F=F, eta=eta, Heta=Heta, U1=parts[0], E_spring=parts[1],
                                     npairs=int(parts[2]))
+    return float(v), grad
+
+
+def veff_grad_fd(osys, R, eps, geom=0, brute=False):
+    """V_eff and -F_eff of eqs (5),(6),(7) as printed: Hessian term by the paper's finite difference
+    [F(R + eps eta) - F(R - eps eta)]/(4 eps).  Returns (veff, grad)."""
+    L = _load()
+    R = np.ascontiguousarray(R, dtype=np.float64)
+    N = R.shape[0]
+    assert R.shape[1:] == (osys.Q, 3)
+    grad = np.zeros_like(R)
+    v = L.orc_veff_grad_fd(osys.ref, C.c_int(N), _p(R), C.c_double(eps), C.c_int(geom), C.c_int(int(brute)), _p(grad))
     return float(v), grad
 
 

@@ -17,7 +17,7 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
           4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
-           "mop_set_timing", "mop_get_timing", "mop_probe_fp32"]
+           "mop_set_timing", "mop_get_timing", "mop_probe_fp32", "mop_eval_veff_grad_fd"]
 
 
 class MopError(RuntimeError):
@@ -73,6 +73,8 @@ def load(build_if_missing=True):
     L.mop_set_timing.argtypes = [C.c_void_p, C.c_int]
     L.mop_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     L.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    L.mop_eval_veff_grad_fd.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]
+    L.mop_eval_veff_grad_fd.restype = C.c_int
     L.mop_probe_fp32.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
@@ -177,6 +179,14 @@ class Mop:
         self._check(self.L.mop_eval_veff_grad(self.ctx, _ptr(R), C.byref(v) if sync else None,
                                               _ptr(grad) if want_grad else None))
         return (v.value if sync else None), (grad if want_grad else None)
+
+    def mop_eval_veff_grad_fd(self, R, eps, sync=True, grad_out=None):
+        """The paper's finite-difference form of the Hessian term (three force passes).  Returns (veff | None, grad)."""
+        R = self._dev(R, (self.N, self.Q, 3))
+        grad = grad_out if grad_out is not None else self.torch.empty_like(R)
+        v = C.c_double(0.0)
+        self._check(self.L.mop_eval_veff_grad_fd(self.ctx, _ptr(R), float(eps), C.byref(v) if sync else None, _ptr(grad)))
+        return (v.value if sync else None), grad
 
     def mop_eval_veff_grad_host(self, R_host, grad_host=None):
         """HOST buffers (torch CPU tensors, ideally pinned, float32 [N][Q][3]).  Returns V_eff; fills grad_host."""

@@ -66,6 +66,8 @@ struct mop_ctx {
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
+    // finite-difference Hessian mode (mop_eval_veff_grad_fd): [nf][Q][3] buffers in original atom order
+    float *d_fdR = 0, *d_fdEta = 0, *d_fdF = 0, *d_fdFp = 0, *d_fdFm = 0;
     // stage timing (mop_set_timing): a ring of event sets, one per evaluation
     bool timing = false;
     cudaEvent_t ev[MOP_TSETS][MOP_NSTAGE + 1];
@@ -135,7 +137,7 @@ static void free_all(mop_ctx *c) {
                     c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
                     c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
                     c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg,       c->d_Rh,
-                    c->d_Gh};
+                    c->d_Gh,      c->d_fdR,      c->d_fdEta,     c->d_fdF,       c->d_fdFp,     c->d_fdFm};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (c->h_energy) cudaFreeHost(c->h_energy);
@@ -249,7 +251,7 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     A(dalloc(&c->d_ctr, 1));
     A(dalloc(&c->d_slots, 1));
     A(dalloc(&c->d_work, 8));
-    A(dalloc(&c->d_energy, 8));
+    A(dalloc(&c->d_energy, 16));   // [0..5] U_lj, U_coul, U_bond, U_angle, E_spring, E_kin; [8..15] scratch
     A(cudaMallocHost((void **)&c->h_energy, 8 * sizeof(double)));
     A(cudaMallocHost((void **)&c->h_ctr, sizeof(MopCounters)));
     A(cudaMallocHost((void **)&c->h_slots, sizeof(unsigned long long)));
@@ -261,7 +263,7 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
         cudaGetLastError();
         return e == cudaErrorMemoryAllocation ? MOP_ERR_OOM : MOP_ERR_CUDA;
     }
-    cudaMemsetAsync(c->d_energy, 0, 8 * sizeof(double), c->st);
+    cudaMemsetAsync(c->d_energy, 0, 16 * sizeof(double), c->st);
     cudaMemsetAsync(c->d_ctr, 0, sizeof(MopCounters), c->st);
     cudaMemsetAsync(c->d_slots, 0, sizeof(unsigned long long), c->st);
     memset(c->h_energy, 0, 8 * sizeof(double));
@@ -517,15 +519,24 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
     return b;
 }
 
-// pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded
-static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false) {
+// pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded.  with_energy = false (displaced
+// configurations of the finite-difference mode): plain force kernel on every bead, energy sums go to scratch
+static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false, bool with_energy = true) {
     const size_t smem = nb_smem(c, c->var_f);
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, nb_pick(NB_ENERGY, c->var_f), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
-    if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    if (with_energy) {
+        LAUNCH(c, nb_pick(NB_ENERGY, c->var_f), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
+        if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+    } else {
+        LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 0, 2));
+    }
     if (timed) t_mark(c, 3);
     const int nterm = c->n_bonds + c->n_angles;
-    if (nterm > 0) LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_F4));
+    if (nterm > 0) {
+        BondedArgs b = bonded_args(c, R, c->d_F4);
+        if (!with_energy) b.energies = c->d_energy + 8;
+        LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, b);
+    }
     if (timed) t_mark(c, 4);
     return MOP_OK;
 }
@@ -597,6 +608,52 @@ extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double 
     if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
     mop_status s = eval_async(c, R_dev, grad_dev);
     if (s) return s;
+    if (veff_out) {
+        if ((s = read_back(c))) return s;
+        *veff_out = c->last_veff;
+    }
+    return MOP_OK;
+}
+
+// The paper's own form of the gradient: Hessian term by finite differences of two displaced force evaluations
+// (eqs (5),(6),(7); PMD kernels 2 and 3).  Three force passes per bead instead of one
+// force pass + one H.eta pass; every displaced configuration gets its own cell list and pair list.
+extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, double eps, double *veff_out, float *grad_dev) {
+    PRECHECK(c);
+    if (!R_dev || !grad_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or grad_dev is NULL");
+    if (!(eps > 0.0) || !std::isfinite(eps)) FAIL(c, MOP_ERR_INVALID_ARG, "need eps > 0");
+    const int nb = c->nf;
+    const size_t per = (size_t)c->Q * 3, tot = per * nb;
+    if (!c->d_fdR) {
+        CK(c, dalloc(&c->d_fdR, tot));
+        CK(c, dalloc(&c->d_fdEta, tot));
+        CK(c, dalloc(&c->d_fdF, tot));
+        CK(c, dalloc(&c->d_fdFp, tot));
+        CK(c, dalloc(&c->d_fdFm, tot));
+    }
+    const MopGrid &g = c->g;
+    const dim3 gq(cdiv(c->Q, 256), nb);
+    CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
+    CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    mop_status s = build_list(c, R_dev, nb);
+    if (s) return s;
+    if ((s = pass_force(c, R_dev, nb))) return s;
+    LAUNCH(c, k_gather3, gq, 256, 0, c->Q, g.S, c->d_slot_of, c->d_F4, c->d_fdF, 1.0f);
+    if (c->N > 1) {
+        LAUNCH(c, k_eta, dim3(cdiv(g.S, 256), nb), 256, 0, c->Q, g.S, R_dev, c->d_perm, c->d_typ, c->d_F4, c->d_ai,
+               c->d_Ki, c->d_et, c->d_energy + 4);
+        LAUNCH(c, k_gather3, gq, 256, 0, c->Q, g.S, c->d_slot_of, c->d_et, c->d_fdEta, 1.0f);
+        for (int sign = 0; sign < 2; sign++) {
+            LAUNCH(c, k_displace, cdiv(tot, 256), 256, 0, tot, sign ? -(float)eps : (float)eps, R_dev, c->d_fdEta, c->d_fdR);
+            CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+            if ((s = build_list(c, c->d_fdR, nb))) return s;
+            if ((s = pass_force(c, c->d_fdR, nb, false, false))) return s;
+            LAUNCH(c, k_gather3, gq, 256, 0, c->Q, g.S, c->d_slot_of, c->d_F4, sign ? c->d_fdFm : c->d_fdFp, 1.0f);
+        }
+    }
+    LAUNCH(c, k_assemble_fd, dim3(cdiv(per, 256), c->N), 256, 0, c->Q, c->N, (float)(1.0 / (4.0 * eps)), c->d_fdF, c->d_fdEta,
+           c->d_fdFp, c->d_fdFm, c->d_Ki, grad_dev);
+    CK(c, cudaGetLastError());
     if (veff_out) {
         if ((s = read_back(c))) return s;
         *veff_out = c->last_veff;

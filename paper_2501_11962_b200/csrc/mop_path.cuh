@@ -121,3 +121,30 @@ __global__ void __launch_bounds__(256) k_verlet(size_t total, int Q, float dt, i
         }
     }
 }
+
+// ---- the paper's finite-difference form of the Hessian term (NEXT-1) ----
+// paper kernel 2: displaced coordinates R^n +- eps eta^n (original atom order, eta in original order)
+__global__ void __launch_bounds__(256) k_displace(size_t total, float eps, const float *__restrict__ R,
+                                                  const float *__restrict__ eta, float *__restrict__ Rd) {
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o < total) Rd[o] = __fmaf_rn(eps, eta[o], R[o]);
+}
+
+// paper kernels 3-6 in gradient form, original atom order:
+//   dV_eff/dR^n = [n = 1: -F^1] + K eta^{n-1} - K eta^n - [F(R^n + eps eta^n) - F(R^n - eps eta^n)] / (4 eps)
+// (eqs (5),(6),(7) with K a_i = 1/2; the bracket replaces -1/2 H^n eta^n)
+__global__ void __launch_bounds__(256) k_assemble_fd(int Q, int N, float inv4eps, const float *__restrict__ F,
+                                                     const float *__restrict__ eta, const float *__restrict__ Fp,
+                                                     const float *__restrict__ Fm, const float *__restrict__ K_i,
+                                                     float *__restrict__ grad) {
+    const int n = blockIdx.y;
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (size_t)Q * 3) return;
+    const float K = K_i[t / 3];
+    const size_t o = (size_t)n * Q * 3 + t;
+    float g = 0.f;
+    if (n == 0) g -= F[t];
+    if (n > 0) g = fmaf(K, eta[o - (size_t)Q * 3], g);
+    if (n < N - 1) g += fmaf(-K, eta[o], -inv4eps * (Fp[o] - Fm[o]));
+    grad[o] = g;
+}

@@ -6,7 +6,8 @@ N = 1, 4, 16, 64, 128 beads on one GPU.
 Per N it prints one JSON line: ms per mop_eval_veff_grad (pair list rebuilt every evaluation, 256 MiB L2 flush
 between timed evaluations, CUDA events), bead-gradient evaluations/s, in-range pair interactions/s, the
 algorithmic FP32 fraction of the H.eta pair kernel, and mop_step throughput (velocity-Verlet PMD steps/s x N,
-integrator kernels included).  The path is the Brownian recursion of BASELINE.json with the force from the
+integrator kernels included), and the time of the paper's finite-difference form of the Hessian term
+(mop_eval_veff_grad_fd, eps = 0.01) with its RMS deviation from the analytic gradient.  The path is the Brownian recursion of BASELINE.json with the force from the
 library's own pass 1 (as in bench.py).  The explicit Euler recursion of the stiff three-site water is not stable
 for much more than ~60 steps at dt = 2 fs (bare +0.41 e sites without LJ), so for N > 32 the
 path is the 32-bead recursion traversed back and forth (every consecutive pair of beads is still one Brownian
@@ -68,6 +69,20 @@ def run(config, N, steps, pmd_steps, device=0):
     b.record()
     torch.cuda.synchronize()
     ms_pmd = a.elapsed_time(b) / pmd_steps   # one evaluation + two half-kick kernels per step (plus the initial evaluation / pmd_steps)
+    # the paper's finite-difference form (three force passes per bead), eps = 0.01
+    ms_fd, fd_vs_analytic = None, None
+    if N > 1:
+        Gf = torch.empty_like(Rd)
+        m.mop_eval_veff_grad_fd(Rd, 0.01, sync=False, grad_out=Gf)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(3):
+            m.mop_eval_veff_grad_fd(Rd, 0.01, sync=False, grad_out=Gf)
+        b.record()
+        torch.cuda.synchronize()
+        ms_fd = a.elapsed_time(b) / 3
+        fd_vs_analytic = float(((Gf - Gd).double().pow(2).sum() / Gd.double().pow(2).sum()).sqrt())
     mem = torch.cuda.max_memory_allocated(dev)
     free, total = torch.cuda.mem_get_info(dev)
     t_h = stages["S5_nb_hvp"] * 1e-3
@@ -77,6 +92,7 @@ def run(config, N, steps, pmd_steps, device=0):
            "stage_ms": {k: round(v, 4) for k, v in stages.items() if k != "evals"},
            "hvp_tflops_algorithmic": (sum(pairs[:n_hvp]) * FLOP_PER_PAIR_HVP / t_h / 1e12) if t_h > 0 else None,
            "ms_per_pmd_step": round(ms_pmd, 4), "pmd_bead_steps_per_sec": round(N / (ms_pmd * 1e-3), 1),
+           "ms_per_eval_fd_form": None if ms_fd is None else round(ms_fd, 4), "fd_vs_analytic_grad_rms_rel": fd_vs_analytic,
            "device_memory_used_gb": round((total - free) / 2 ** 30, 2), "veff": st["veff"]}
     m.close()
     return out

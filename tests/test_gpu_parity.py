@@ -179,6 +179,29 @@ def test_config4_full_size_bench_configuration(B, oracle):
     m.close()
 
 
+# --------------------------------------------------------------------------- NEXT-1: the paper's finite-difference form
+TOL_FD = 1e-3   # FP32 force rounding (~1e-6 |F|, see BASELINE.md parity rows) enters twice and is divided by 4 eps:
+                # sqrt(2) 1e-6 |F|_rms / (4 eps |G|_rms) ~ 4e-5 at eps = 0.01 with |F| ~ |G|; 1e-3 leaves room for the
+                # few coordinates whose FP32 displaced position rounds differently from FP64 eta (1 ulp)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "chain", "lj_n1"])
+def test_fd_form_matches_oracle_fd_form(B, oracle, name):
+    """mop_eval_veff_grad_fd (eqs 5-7 as printed, three force passes) against the oracle's own FD form at the same
+    eps, and -- loosely -- against the analytic form (they differ by O(eps^2) and by pairs crossing r_c, G9)."""
+    s, o, R = case(oracle, name)
+    eps = 0.01
+    m = B.Mop(s, s.n_beads)
+    v, g = m.mop_eval_veff_grad_fd(R, eps)
+    v_ref, g_ref = oracle.veff_grad_fd(o, R.astype(np.float64), float(np.float32(eps)), geom=1, brute=True)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_FD
+    v2, g2 = m.mop_eval_veff_grad(R)
+    assert abs(v - v2) <= 1e-7 * abs(v2)
+    assert H.rms_rel(g.cpu().numpy(), g2.cpu().numpy()) <= 5e-2
+    m.close()
+
+
 def test_async_eval_matches_sync_and_repeats(B, oracle):
     """veff_out = NULL leaves the value in the context; repeated evaluations agree to float-atomic noise."""
     s, o, R = case(oracle, "c2")

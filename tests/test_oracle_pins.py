@@ -207,6 +207,36 @@ def test_P5_paper_equations_5_6_7(oracle):
         assert H.rms_rel(-G[n], Feff[n]) < 5e-6
 
 
+def test_P5b_fd_form_of_the_oracle(oracle):
+    """veff_grad_fd is eqs (5),(6),(7) as printed.  Pinned two ways: (i) against the equations retyped here with
+    the oracle's plain force (no shared arithmetic beyond F); (ii) against the analytic gradient, from which it may
+    differ only by the O(eps^2) truncation of the central difference (and by pairs crossing r_c, G9: none here)."""
+    s = _systems()[3]
+    o, R = _tiny_path(oracle, s, 5)
+    N = R.shape[0]
+    m = s.mass.astype(float)[:, None]
+    K = m * s.nu / (2 * s.dt_path)
+    a = s.dt_path / (m * s.nu)
+    force = lambda X: oracle.bead(o, X, geom=0, brute=True)["F"]
+    F = [force(R[n]) for n in range(N)]
+    eps = 0.02
+    Feff = np.zeros_like(R)
+    for n in range(N - 1):
+        eta = R[n + 1] - R[n] - a * F[n]
+        br = (force(R[n] + eps * eta) - force(R[n] - eps * eta)) / (4 * eps)
+        Feff[n] = (0.5 * F[0] + K * (R[1] - R[0]) + br) if n == 0 else \
+            (-K * (2 * R[n] - R[n - 1] - R[n + 1]) + 0.5 * (F[n - 1] - F[n]) + br)
+    Feff[N - 1] = -K * (R[N - 1] - R[N - 2]) + 0.5 * F[N - 2]
+    v_fd, G_fd = oracle.veff_grad_fd(o, R, eps, geom=0, brute=True)
+    v, G = oracle.veff_grad(o, R, geom=0, brute=True)
+    assert v_fd == pytest.approx(v, rel=1e-13)
+    assert H.rms_rel(-G_fd, Feff) < 1e-12
+    assert H.rms_rel(G_fd, G) < 1e-8      # eps |eta| ~ 1e-4 nm: truncation ~1e-12, and no pair crosses r_c here (G9)
+    # N = 1: plain force
+    v1, G1 = oracle.veff_grad_fd(o, R[:1], eps, geom=0, brute=True)
+    assert np.allclose(G1[0], -F[0], rtol=1e-13, atol=1e-13)
+
+
 # ---------------------------------------------------------------- P6 / P7 invariants
 @pytest.mark.parametrize("idx", range(3))
 def test_P6_newton_third_law_and_translation(oracle, idx):

@@ -173,6 +173,21 @@ mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float *s_dev, flo
  * call mop_debug_get / mop_debug_pairs describe the last displaced configuration.  Errors: INVALID_ARG, OOM, CUDA. */
 mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, double eps, double *veff_out, float *grad_dev);
 
+/* Path MD in the canonical ensemble (the paper's NVT validation and scaling runs: "Langevin thermostat ... damping
+ * coefficient 0.25 fs^-1" at 310 K, Fig. 4b).  The paper does not give the discretisation;
+ * reading G19: each step is the velocity-Verlet step of mop_step followed by the exact Ornstein-Uhlenbeck
+ * velocity update  v <- c v + sqrt((1 - c^2) k_B T / m_i) xi,  c = exp(-gamma dt_pmd),  k_B = 0.0083144626 kJ/mol/K,
+ * xi ~ N(0,1) drawn from a counter-based generator keyed by (seed, step0 + step index, index of the coordinate in
+ * [N][Q][3]), so a run can be replayed and continued (pass step0 = steps already done).  gamma (1/ps) >= 0; gamma = 0
+ * is mop_step.  E_kin in mop_get_stats is taken after the thermostat update of the last step.  Asynchronous. */
+mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
+                             double temperature, unsigned long long seed, unsigned long long step0);
+
+/* Debug: the 64 raw bits of the thermostat's generator for (seed, step, idx), idx = 0..n-1, to HOST memory
+ * (compared bit for bit with the oracle's independent implementation).  Synchronises. */
+mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, unsigned long long step, int n,
+                                unsigned long long *host_out);
+
 /* Measurement aid, not part of the path: achieved FP32 rate (TFLOP/s, FMA = 2 flop) of dependent-free FMA streams
  * on all SMs of `device`, timed with CUDA events on the default stream (synchronises):
  *   out[0] scalar FFMA with a reused operand (the nominal 128 lanes/clk/SM peak of DESIGN.md section 5),

@@ -23,7 +23,8 @@
  *   O5 grad V_eff      derivative of eq. (3); equals -(eqs 5,6,7)
  *   O5-FD              the same gradient with the paper's own finite-difference
  *                      Hessian term, eqs (5),(6),(7) as printed (orc_veff_grad_fd)
- *   O6 integrator      velocity Verlet on eq. (4)
+ *   O6 integrator      velocity Verlet on eq. (4); with the
+ *                      Langevin thermostat of the NVT runs (reading G19): orc_step_langevin
  *
  * Geometry modes (argument `geom`):
  *   0  pure FP64: positions as given, minimum image and r < r_c in double.
@@ -777,6 +778,62 @@ void orc_step(const orc_system *s, int N, double *R, double *V, double dt, int n
         for (size_t o = 0; o < tot; o++) {
             double m = (double)s->mass[(o / 3) % (size_t)Q];
             V[o] += 0.5 * dt * (-G[o]) / m;
+        }
+    }
+    free(G);
+}
+
+/* ------------------------------------------------------------------ */
+/* O6-NVT: path MD with a Langevin thermostat ("the Langevin */
+/* thermostat, as implemented in GROMACS, damping coefficient 0.25 fs^-1", */
+/* Fig. 4b).  The paper gives no discretisation; reading G19 */
+/* (DESIGN.md): one velocity-Verlet step of eq. (4), then the exact        */
+/* Ornstein-Uhlenbeck velocity update over dt                              */
+/*    v <- c v + sqrt((1 - c^2) kT / m) xi,   c = exp(-gamma dt),          */
+/* xi ~ N(0,1) from a counter-based generator keyed by (seed, step, index  */
+/* of the coordinate in [N][Q][3]): 64-bit mix -> two 32-bit uniforms ->   */
+/* Box-Muller.  gamma = 0 reproduces orc_step exactly.                     */
+/* ------------------------------------------------------------------ */
+static uint64_t orc_mix64(uint64_t z) { /* SplitMix64 finaliser (Steele, Lea, Flood 2014) */
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+/* the 64 random bits of (seed, step, idx) */
+uint64_t orc_noise_bits(uint64_t seed, uint64_t step, uint64_t idx) {
+    return orc_mix64(orc_mix64(seed + 0x9E3779B97F4A7C15ULL * (step + 1)) ^ (idx * 0xD1342543DE82EF95ULL + 1));
+}
+double orc_noise_normal(uint64_t seed, uint64_t step, uint64_t idx) {
+    uint64_t b = orc_noise_bits(seed, step, idx);
+    double u1 = ((double)(uint32_t)(b >> 32) + 0.5) / 4294967296.0; /* in (0,1) */
+    double u2 = ((double)(uint32_t)b + 0.5) / 4294967296.0;
+    return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925 * u2);
+}
+/* energies[3*(n_steps+1)] as in orc_step (kinetic energy after the thermostat update) */
+void orc_step_langevin(const orc_system *s, int N, double *R, double *V, double dt, int n_steps, double gamma,
+                       double kT, uint64_t seed, uint64_t step0, int geom, int brute, double *energies) {
+    int Q = s->n_atoms;
+    size_t tot = 3 * (size_t)Q * (size_t)N;
+    double *G = (double *)malloc(sizeof(double) * tot);
+    double veff = orc_veff_grad(s, N, R, geom, brute, G, NULL, NULL, NULL, NULL);
+    double c = exp(-gamma * dt), amp = sqrt(1.0 - c * c);
+    for (int st = 0; st <= n_steps; st++) {
+        if (energies) {
+            double ek = 0.0;
+            for (size_t o = 0; o < tot; o++) ek += 0.5 * (double)s->mass[(o / 3) % (size_t)Q] * V[o] * V[o];
+            energies[3 * st] = veff, energies[3 * st + 1] = ek, energies[3 * st + 2] = veff + ek;
+        }
+        if (st == n_steps) break;
+        for (size_t o = 0; o < tot; o++) {
+            double m = (double)s->mass[(o / 3) % (size_t)Q];
+            V[o] += 0.5 * dt * (-G[o]) / m;
+            R[o] += dt * V[o];
+        }
+        veff = orc_veff_grad(s, N, R, geom, brute, G, NULL, NULL, NULL, NULL);
+        for (size_t o = 0; o < tot; o++) {
+            double m = (double)s->mass[(o / 3) % (size_t)Q];
+            V[o] += 0.5 * dt * (-G[o]) / m;
+            if (gamma > 0.0) V[o] = c * V[o] + amp * sqrt(kT / m) * orc_noise_normal(seed, step0 + (uint64_t)st, (uint64_t)o);
         }
     }
     free(G);

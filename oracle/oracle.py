@@ -53,6 +53,8 @@ def _load():
         L.orc_bead.restype = C.c_long
         L.orc_veff_grad.restype = C.c_double
         L.orc_veff_grad_fd.restype = C.c_double
+        L.orc_noise_normal.restype = C.c_double
+        L.orc_noise_bits.restype = C.c_uint64
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -221,4 +223,29 @@ def step(osys, R, V, dt, n_steps, geom=0, brute=False):
     en = np.zeros((n_steps + 1, 3))
     L.orc_step(osys.ref, C.c_int(N), _p(R), _p(V), C.c_double(dt), C.c_int(n_steps), C.c_int(geom),
                C.c_int(int(brute)), _p(en))
+    return R, V, en
+
+
+KB = 0.0083144626   # kJ mol^-1 K^-1
+
+
+def noise_bits(seed, step, idx):
+    """The 64 random bits of the counter (seed, step, idx) of the thermostat's generator."""
+    return int(_load().orc_noise_bits(C.c_uint64(seed), C.c_uint64(step), C.c_uint64(idx)))
+
+
+def noise_normal(seed, step, idx):
+    return float(_load().orc_noise_normal(C.c_uint64(seed), C.c_uint64(step), C.c_uint64(idx)))
+
+
+def step_langevin(osys, R, V, dt, n_steps, gamma, temperature, seed=0, step0=0, geom=0, brute=False):
+    """Velocity Verlet + exact Ornstein-Uhlenbeck velocity update (reading G19).  Returns (R, V, energies)."""
+    L = _load()
+    R = np.array(R, dtype=np.float64, order="C", copy=True)
+    V = np.array(V, dtype=np.float64, order="C", copy=True)
+    N = R.shape[0]
+    en = np.zeros((n_steps + 1, 3))
+    L.orc_step_langevin(osys.ref, C.c_int(N), _p(R), _p(V), C.c_double(dt), C.c_int(n_steps), C.c_double(gamma),
+                        C.c_double(KB * temperature), C.c_uint64(seed), C.c_uint64(step0), C.c_int(geom),
+                        C.c_int(int(brute)), _p(en))
     return R, V, en

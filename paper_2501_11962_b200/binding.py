@@ -17,7 +17,8 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
           4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
-           "mop_set_timing", "mop_get_timing", "mop_probe_fp32", "mop_eval_veff_grad_fd"]
+           "mop_set_timing", "mop_get_timing", "mop_probe_fp32", "mop_eval_veff_grad_fd",
+           "mop_step_langevin", "mop_debug_noise_bits"]
 
 
 class MopError(RuntimeError):
@@ -75,6 +76,11 @@ def load(build_if_missing=True):
     L.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
     L.mop_eval_veff_grad_fd.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]
     L.mop_eval_veff_grad_fd.restype = C.c_int
+    L.mop_step_langevin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
+                                    C.c_uint64, C.c_uint64]
+    L.mop_step_langevin.restype = C.c_int
+    L.mop_debug_noise_bits.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p]
+    L.mop_debug_noise_bits.restype = C.c_int
     L.mop_probe_fp32.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
@@ -217,6 +223,18 @@ class Mop:
         assert R.is_cuda and V.is_cuda and R.is_contiguous() and V.is_contiguous()
         assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
         self._check(self.L.mop_step(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps)))
+
+    def mop_step_langevin(self, R, V, dt_pmd, n_steps, gamma, temperature, seed=0, step0=0):
+        """In-place velocity Verlet + exact OU thermostat update on torch cuda tensors R, V [N][Q][3] float32."""
+        assert R.is_cuda and V.is_cuda and R.is_contiguous() and V.is_contiguous()
+        assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
+        self._check(self.L.mop_step_langevin(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps), float(gamma),
+                                             float(temperature), int(seed), int(step0)))
+
+    def mop_debug_noise_bits(self, seed, step, n):
+        out = np.empty(n, np.uint64)
+        self._check(self.L.mop_debug_noise_bits(self.ctx, int(seed), int(step), int(n), out.ctypes.data_as(C.c_void_p)))
+        return out
 
     def mop_force_hvp(self, R1, s=None):
         """Physical force (and H.s for a direction s) of one configuration [Q][3].  Returns (F, Hs) tensors."""

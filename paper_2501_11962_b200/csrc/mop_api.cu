@@ -725,6 +725,53 @@ extern "C" mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt
     return MOP_OK;
 }
 
+// path MD with the Langevin thermostat of the paper's NVT runs: velocity Verlet, then the exact OU velocity update
+extern "C" mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
+                                        double temperature, unsigned long long seed, unsigned long long step0) {
+    PRECHECK(c);
+    if (!R_dev || !V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or V_dev is NULL");
+    if (n_steps < 0 || !(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
+    if (!(gamma >= 0.0) || !(temperature >= 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need gamma >= 0 and temperature >= 0");
+    const size_t total = (size_t)c->N * c->Q * 3;
+    if (!c->d_G) CK(c, dalloc(&c->d_G, total));
+    mop_status s = eval_async(c, R_dev, c->d_G);
+    if (s) return s;
+    const unsigned nblk = cdiv(total, 256);
+    const double cc = exp(-gamma * dt_pmd);
+    const float amp = (float)sqrt((1.0 - cc * cc) * 0.0083144626 * temperature);   // k_B in kJ mol^-1 K^-1
+    const bool ou = gamma > 0.0;
+    for (int it = 0; it < n_steps; it++) {
+        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
+               (double *)nullptr);
+        if ((s = eval_async(c, R_dev, c->d_G))) return s;
+        const bool last = it == n_steps - 1;
+        if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
+        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
+               (last && !ou) ? c->d_energy + 5 : (double *)nullptr);
+        if (ou)
+            LAUNCH(c, k_ou, nblk, 256, 0, total, c->Q, (float)cc, amp, seed, step0 + (unsigned long long)it, c->d_inv_mass,
+                   c->d_mass, V_dev, last ? c->d_energy + 5 : (double *)nullptr);
+    }
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+// debug: raw bits of the thermostat's counter-based generator for idx = 0..n-1 (HOST output)
+extern "C" mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, unsigned long long step, int n,
+                                           unsigned long long *host_out) {
+    PRECHECK(c);
+    if (n < 0 || (n > 0 && !host_out)) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_noise_bits: bad argument");
+    if (n == 0) return MOP_OK;
+    unsigned long long *d = nullptr;
+    CK(c, dalloc(&d, (size_t)n));
+    LAUNCH(c, k_noise_bits, cdiv(n, 256), 256, 0, n, seed, step, d);
+    cudaError_t e = cudaMemcpyAsync(host_out, d, (size_t)n * 8, cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    cudaFree(d);
+    CK(c, e);
+    return MOP_OK;
+}
+
 extern "C" mop_status mop_get_stats(mop_ctx *c, double out[16]) {
     PRECHECK(c);
     if (!out) FAIL(c, MOP_ERR_INVALID_ARG, "out is NULL");

@@ -148,3 +148,55 @@ __global__ void __launch_bounds__(256) k_assemble_fd(int Q, int N, float inv4eps
     if (n < N - 1) g += fmaf(-K, eta[o], -inv4eps * (Fp[o] - Fm[o]));
     grad[o] = g;
 }
+
+// ---- Langevin thermostat of the NVT runs (NEXT-2; reading G19 of DESIGN.md) ----
+// Counter-based noise: 64 bits from (seed, step, index of the coordinate in [N][Q][3]) by two SplitMix64
+// finalisers, two 32-bit uniforms, Box-Muller.  The integer part is bit-identical to the oracle's generator
+// (written independently there); the transcendental part is FP32 here and FP64 there.
+__device__ __forceinline__ unsigned long long mop_mix64(unsigned long long z) {
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+__device__ __forceinline__ unsigned long long mop_noise_bits(unsigned long long seed, unsigned long long step,
+                                                             unsigned long long idx) {
+    return mop_mix64(mop_mix64(seed + 0x9E3779B97F4A7C15ULL * (step + 1ULL)) ^ (idx * 0xD1342543DE82EF95ULL + 1ULL));
+}
+__device__ __forceinline__ float mop_noise_normal(unsigned long long seed, unsigned long long step, unsigned long long idx) {
+    const unsigned long long b = mop_noise_bits(seed, step, idx);
+    const double u1 = ((double)(unsigned)(b >> 32) + 0.5) * (1.0 / 4294967296.0);   // exact in FP64, in (0,1)
+    const float u2 = (float)(((double)(unsigned)b + 0.5) * (1.0 / 4294967296.0));
+    return sqrtf(-2.0f * (float)log(u1)) * cospif(2.0f * u2);
+}
+
+// exact Ornstein-Uhlenbeck velocity update over dt: v <- c v + sqrt((1 - c^2) kT / m) xi  (+ kinetic energy)
+__global__ void __launch_bounds__(256) k_ou(size_t total, int Q, float c, float amp, unsigned long long seed,
+                                            unsigned long long step, const float *__restrict__ inv_m,
+                                            const float *__restrict__ m, float *__restrict__ V,
+                                            double *__restrict__ e_kin) {
+    const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double ek = 0.0;
+    if (o < total) {
+        const int i = (int)((o / 3) % (size_t)Q);
+        const float v = fmaf(c, V[o], amp * sqrtf(inv_m[i]) * mop_noise_normal(seed, step, o));
+        V[o] = v;
+        if (e_kin) ek = 0.5 * (double)m[i] * (double)v * (double)v;
+    }
+    if (e_kin) {
+        __shared__ double sh[8];
+        ek = mop_warp_sum_d(ek);
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = ek;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            double v = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : 0.0;
+            v = mop_warp_sum_d(v);
+            if (threadIdx.x == 0) atomicAdd(e_kin, v);
+        }
+    }
+}
+
+// debug: the generator's raw bits for idx = 0..n-1 (bit-exact comparison with the oracle)
+__global__ void k_noise_bits(int n, unsigned long long seed, unsigned long long step, unsigned long long *out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = mop_noise_bits(seed, step, (unsigned long long)i);
+}

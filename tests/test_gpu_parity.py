@@ -257,6 +257,63 @@ def test_nve_energy_conservation(B, oracle):
     m.close()
 
 
+# --------------------------------------------------------------------------- NEXT-2: Langevin thermostat (G19)
+def test_thermostat_noise_bits_bit_exact(B, oracle):
+    s = W.config1(n_beads=2)
+    m = B.Mop(s, 2)
+    for seed, step in ((0, 0), (7, 3), (2 ** 63 + 5, 2 ** 40)):
+        got = m.mop_debug_noise_bits(seed, step, 4096)
+        ref = np.array([oracle.noise_bits(seed, step, i) for i in range(4096)], dtype=np.uint64)
+        assert np.array_equal(got, ref)
+    m.close()
+
+
+@pytest.mark.parametrize("name", ["c1", "chain"])
+def test_langevin_step_matches_oracle(B, oracle, name):
+    import torch
+    s, o, R = case(oracle, name)
+    rng = np.random.default_rng(21)
+    sd = np.sqrt(W.KB * s.temperature / s.mass.astype(np.float64))
+    V0 = (rng.normal(0, 1, R.shape) * sd[None, :, None]).astype(np.float32)
+    m = B.Mop(s, s.n_beads)
+    Rg, Vg = torch.tensor(R, device="cuda"), torch.tensor(V0, device="cuda")
+    nst, dt, gamma = 5, 0.001, 250.0          # the paper's damping: 0.25 fs^-1 = 250 ps^-1
+    m.mop_step_langevin(Rg, Vg, dt, nst, gamma, s.temperature, seed=9, step0=100)
+    R_ref, V_ref, en = oracle.step_langevin(o, R.astype(np.float64), V0.astype(np.float64), dt, nst, gamma,
+                                            s.temperature, seed=9, step0=100, geom=1, brute=True)
+    dR_ref = R_ref - R.astype(np.float64)
+    dR = Rg.cpu().numpy().astype(np.float64) - R.astype(np.float64)
+    assert H.rms_rel(dR, dR_ref) <= 2e-3        # FP32 positions, as in test_step_matches_oracle
+    assert H.rms_rel(Vg.cpu().numpy(), V_ref) <= 1e-4
+    ek = m.mop_get_stats()["E_kin"]
+    assert abs(ek - en[-1, 1]) <= 1e-4 * en[-1, 1]
+    # gamma = 0 is mop_step
+    Ra, Va = torch.tensor(R, device="cuda"), torch.tensor(V0, device="cuda")
+    Rb, Vb = torch.tensor(R, device="cuda"), torch.tensor(V0, device="cuda")
+    m.mop_step(Ra, Va, dt, 2)
+    m.mop_step_langevin(Rb, Vb, dt, 2, 0.0, s.temperature)
+    assert H.rms_rel(Vb.cpu().numpy(), Va.cpu().numpy()) <= 1e-5 and H.rms_rel(Rb.cpu().numpy(), Ra.cpu().numpy()) <= 1e-7
+    m.close()
+
+
+def test_nvt_temperature_stays_at_target(B, oracle):
+    """Fig. 4b analogue: kinetic temperature of the polymer under the thermostat, from rest."""
+    import torch
+    s, o, R = case(oracle, "c1")
+    m = B.Mop(s, s.n_beads)
+    Rg = torch.tensor(R, device="cuda")
+    Vg = torch.zeros_like(Rg)
+    T, dt, gamma = s.temperature, 0.0005, 100.0
+    m.mop_step_langevin(Rg, Vg, dt, 150, gamma, T, seed=1)
+    tk, done = [], 150
+    for _ in range(12):
+        m.mop_step_langevin(Rg, Vg, dt, 25, gamma, T, seed=1, step0=done)
+        done += 25
+        tk.append(2.0 * m.mop_get_stats()["E_kin"] / (R.size * W.KB))
+    assert abs(np.mean(tk) / T - 1.0) < 0.03      # 24,576 degrees of freedom, 12 samples
+    m.close()
+
+
 # --------------------------------------------------------------------------- degenerate inputs and errors
 def test_edge_cases(B, oracle):
     # two atoms, one pair; then out of range

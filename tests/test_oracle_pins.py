@@ -350,6 +350,68 @@ def test_P12_velocity_verlet_invariants(oracle):
     assert np.abs(Vb + V).max() < 1e-6
 
 
+# ---------------------------------------------------------------- P14 Langevin thermostat (NEXT-2, reading G19)
+def test_P14_noise_generator_statistics(oracle):
+    """The counter-based generator: unbiased bits, N(0,1) moments, no correlation along idx or step."""
+    bits = np.array([oracle.noise_bits(7, 3, i) for i in range(20000)], dtype=np.uint64)
+    for b in (0, 1, 17, 31, 32, 47, 63):
+        assert abs(float(((bits >> np.uint64(b)) & np.uint64(1)).mean()) - 0.5) < 0.012
+    assert len(np.unique(bits)) == len(bits)
+    x = np.array([[oracle.noise_normal(11, st, i) for i in range(20000)] for st in range(3)])
+    assert abs(x.mean()) < 0.015 and abs(x.var() - 1.0) < 0.02
+    assert abs((x ** 4).mean() - 3.0) < 0.15 and abs((x ** 3).mean()) < 0.05
+    assert abs(np.mean(x[0, :-1] * x[0, 1:])) < 0.02 and abs(np.mean(x[0] * x[1])) < 0.02
+    assert oracle.noise_normal(11, 0, 5) != oracle.noise_normal(12, 0, 5)          # the seed matters
+    assert oracle.noise_normal(11, 2, 5) == x[2, 5]                                # and it is a pure function
+
+
+def test_P14_gamma_zero_is_velocity_verlet(oracle):
+    s = H.lj_cluster(32)
+    o, R = _tiny_path(oracle, s, 3)
+    V = np.random.default_rng(4).normal(0, 0.3, R.shape)
+    R1, V1, e1 = oracle.step(o, R, V, 0.001, 7, geom=0, brute=True)
+    R2, V2, e2 = oracle.step_langevin(o, R, V, 0.001, 7, 0.0, 120.0, seed=5, geom=0, brute=True)
+    assert np.array_equal(R1, R2) and np.array_equal(V1, V2) and np.array_equal(e1, e2)
+
+
+def test_P14_free_particles_follow_the_exact_ornstein_uhlenbeck_law(oracle):
+    """No forces (eps = 0, q = 0, N = 1, so V_eff = 0): v_n is an exact OU chain with c = exp(-gamma dt):
+    Var(v_n) = (kT/m)(1 - c^(2n)) from rest, lag-1 correlation c in the stationary state."""
+    n = 1500
+    rng = np.random.default_rng(1)
+    m = np.linspace(4.0, 40.0, n)
+    s = H.make_system("free", [6.0] * 3, rng.uniform(0, 6, (n, 3)), m, np.zeros(n), np.zeros(n, int), [0.3], [0.0],
+                      r_cut=1.0, eps_rf=0.0, T=300.0)
+    o = oracle.OracleSystem(s)
+    R0, V0 = s.R1[None].astype(float), np.zeros((1, n, 3))
+    T, dt, gamma = 300.0, 0.001, 200.0
+    c = np.exp(-gamma * dt)
+    kT_m = oracle.KB * T / m[None, :, None]
+    R1, V1, _ = oracle.step_langevin(o, R0, V0, dt, 3, gamma, T, seed=2, geom=0, brute=False)
+    r = (V1 ** 2 / kT_m).mean()
+    assert abs(r - (1 - c ** 6)) < 4 * (1 - c ** 6) * np.sqrt(2.0 / (3 * n))
+    Ra, Va, _ = oracle.step_langevin(o, R0, V0, dt, 40, gamma, T, seed=2, geom=0, brute=False)        # 8 relaxation times
+    Rb, Vb, _ = oracle.step_langevin(o, Ra, Va, dt, 1, gamma, T, seed=2, step0=40, geom=0, brute=False)
+    assert abs((Va ** 2 / kT_m).mean() - 1.0) < 4 * np.sqrt(2.0 / (3 * n))
+    assert abs((Va * Vb / kT_m).mean() - c) < 4 / np.sqrt(3 * n)
+    # continuing with step0 replays the same stream as one longer call
+    Rc, Vc, _ = oracle.step_langevin(o, R0, V0, dt, 41, gamma, T, seed=2, geom=0, brute=False)
+    assert np.allclose(Vc, Vb, rtol=0, atol=1e-12) and np.allclose(Rc, Rb, rtol=0, atol=1e-12)
+
+
+def test_P14_nvt_temperature_of_an_interacting_path(oracle):
+    """Fig. 4b analogue: the kinetic temperature of the polymer under the thermostat stays at T."""
+    s = H.lj_cluster(32)
+    o, R = _tiny_path(oracle, s, 4)
+    T = 120.0
+    V = np.zeros_like(R)
+    Ra, Va, _ = oracle.step_langevin(o, R, V, 0.0005, 300, 100.0, T, seed=3, geom=0, brute=True)     # equilibrate
+    Rb, Vb, en = oracle.step_langevin(o, Ra, Va, 0.0005, 1500, 100.0, T, seed=3, step0=300, geom=0, brute=True)
+    dof = R.size
+    t_kin = 2.0 * en[:, 1] / (dof * oracle.KB)
+    assert abs(t_kin.mean() / T - 1.0) < 0.04
+
+
 # ---------------------------------------------------------------- P13 + G8 neighbour sets
 @pytest.mark.parametrize("mk", ["c1", "c2", "tiny", "edge"])
 def test_P13_cell_list_equals_brute_force(oracle, mk):

@@ -188,6 +188,23 @@ mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, double dt_p
 mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, unsigned long long step, int n,
                                 unsigned long long *host_out);
 
+/* Metadynamics of paths: a history-dependent bias V(S) = sum_k height exp(-(S - S_k)^2 / (2 sigma^2))
+ * on the end-to-end collective variable S_e2e = s(R^N) - s(R^1) (eq. 8), with s(R) = the distance between the centres of mass
+ * of two atom groups ("the center of mass of the ligand and the binding pocket"; minimum image of the COM
+ * difference; each group must be whole in the caller's coordinates).  While a bias is set, every evaluation that writes a
+ * gradient (mop_eval_veff_grad, _host, mop_step, mop_step_langevin; not mop_eval_veff_grad_fd) adds dV/dR^1 and dV/dR^N to
+ * it -- the CV touches the first and last bead only -- and mop_step / mop_step_langevin deposit a hill at the current S_e2e
+ * every `pace` steps (PAPER.md:155 deposits one every 500; 0: never).  veff_out stays eq. (3) without V(S).
+ * group_a, group_b: HOST index arrays (copied).  n_a = n_b = 0 switches the bias off.  Setting a bias clears the hills.
+ * Errors: INVALID_ARG (empty group, index out of range, sigma <= 0, n_beads < 2), OOM, CUDA. */
+mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, const int *group_b, int n_b, double sigma, double height,
+                        int pace);
+/* Deposits one hill centred at s_center by hand (at most 65536 hills; OOM beyond).  Synchronises. */
+mop_status mop_add_hill(mop_ctx *c, double s_center);
+/* State of the bias at the last evaluation (synchronises): out[0] S_e2e, out[1] s(R^1), out[2] s(R^N), out[3] V(S),
+ * out[4] dV/dS, out[5] number of hills; hills_host (may be NULL) receives up to cap hill centres, *n_hills their number. */
+mop_status mop_get_bias(mop_ctx *c, double out[8], double *hills_host, int cap, int *n_hills);
+
 /* Measurement aid, not part of the path: achieved FP32 rate (TFLOP/s, FMA = 2 flop) of dependent-free FMA streams
  * on all SMs of `device`, timed with CUDA events on the default stream (synchronises):
  *   out[0] scalar FFMA with a reused operand (the nominal 128 lanes/clk/SM peak of DESIGN.md section 5),

@@ -26,6 +26,9 @@
  *   O6 integrator      velocity Verlet on eq. (4); with the
  *                      Langevin thermostat of the NVT runs (reading G19): orc_step_langevin
  *
+ *   O7 MoP bias        S_e2e = s(R^N) - s(R^1) (eq. 8), s = COM distance of
+ *                      two atom groups, V(S) a sum of Gaussians
+ *
  * Geometry modes (argument `geom`):
  *   0  pure FP64: positions as given, minimum image and r < r_c in double.
  *      Used by the pins (finite differences, invariants, closed forms).
@@ -837,6 +840,75 @@ void orc_step_langevin(const orc_system *s, int N, double *R, double *V, double 
         }
     }
     free(G);
+}
+
+/* ------------------------------------------------------------------ */
+/* O7: the metadynamics-of-paths bias.            */
+/*   CV   S_e2e = s(R^N) - s(R^1)                      eq. (8)          */
+/*   s(R) = distance between the centres of mass of two atom groups     */
+/*          ("the distance between the center of mass of the ligand and */
+/*          the binding pocket"), minimum image of the    */
+/*          COM difference; every group is whole in the given coords    */
+/*   V(S) = sum_k w exp(-(S - S_k)^2 / (2 sigma^2))   (PAPER.md:80-82:  */
+/*          "a sum of Gaussian functions deposited along the CV")       */
+/* ------------------------------------------------------------------ */
+/* s(X) for one bead X [Q][3]; dsdr [Q][3] (may be NULL) receives ds/dr_i (zero off the groups) */
+double orc_cv_com_distance(const orc_system *s, const double *X, const int *ga, int na, const int *gb, int nb,
+                           double *dsdr) {
+    double ca[3] = {0, 0, 0}, cb[3] = {0, 0, 0}, ma = 0.0, mb = 0.0, d[3];
+    for (int k = 0; k < na; k++) {
+        double m = (double)s->mass[ga[k]];
+        ma += m;
+        for (int q = 0; q < 3; q++) ca[q] += m * X[3 * (size_t)ga[k] + q];
+    }
+    for (int k = 0; k < nb; k++) {
+        double m = (double)s->mass[gb[k]];
+        mb += m;
+        for (int q = 0; q < 3; q++) cb[q] += m * X[3 * (size_t)gb[k] + q];
+    }
+    double r2 = 0.0;
+    for (int q = 0; q < 3; q++) {
+        double L = (double)s->box[q];
+        d[q] = ca[q] / ma - cb[q] / mb;
+        d[q] -= L * floor(d[q] / L + 0.5);
+        r2 += d[q] * d[q];
+    }
+    double r = sqrt(r2);
+    if (dsdr) {
+        memset(dsdr, 0, sizeof(double) * 3 * (size_t)s->n_atoms);
+        if (r > 0.0) {
+            for (int k = 0; k < na; k++)
+                for (int q = 0; q < 3; q++) dsdr[3 * (size_t)ga[k] + q] += (double)s->mass[ga[k]] / ma * d[q] / r;
+            for (int k = 0; k < nb; k++)
+                for (int q = 0; q < 3; q++) dsdr[3 * (size_t)gb[k] + q] -= (double)s->mass[gb[k]] / mb * d[q] / r;
+        }
+    }
+    return r;
+}
+/* V(S_e2e) of a path R [N][Q][3] (N >= 2); grad_add [N][Q][3] (may be NULL) receives dV/dR^n (zero on the interior
+ * beads: the CV touches beads 1 and N only); out[3] = {S_e2e, s(R^1), s(R^N)} (may be NULL).  Returns V.            */
+double orc_bias(const orc_system *s, int N, const double *R, const int *ga, int na, const int *gb, int nb,
+                const double *hills, int nh, double sigma, double w, double *grad_add, double *out) {
+    size_t bead = 3 * (size_t)s->n_atoms;
+    double *d1 = (double *)malloc(sizeof(double) * bead), *dN = (double *)malloc(sizeof(double) * bead);
+    double s1 = orc_cv_com_distance(s, R, ga, na, gb, nb, d1);
+    double sN = orc_cv_com_distance(s, R + bead * (size_t)(N - 1), ga, na, gb, nb, dN);
+    double S = sN - s1, V = 0.0, dVdS = 0.0;
+    for (int k = 0; k < nh; k++) {
+        double u = (S - hills[k]) / sigma, e = w * exp(-0.5 * u * u);
+        V += e;
+        dVdS += -e * u / sigma;
+    }
+    if (grad_add) {
+        memset(grad_add, 0, sizeof(double) * bead * (size_t)N);
+        for (size_t o = 0; o < bead; o++) {
+            grad_add[o] += -dVdS * d1[o];                          /* dS/dR^1 = -ds/dR^1 */
+            grad_add[bead * (size_t)(N - 1) + o] += dVdS * dN[o];  /* dS/dR^N = +ds/dR^N */
+        }
+    }
+    if (out) out[0] = S, out[1] = s1, out[2] = sN;
+    free(d1), free(dN);
+    return V;
 }
 
 int orc_num_threads(void) {

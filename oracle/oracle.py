@@ -54,6 +54,8 @@ def _load():
         L.orc_veff_grad.restype = C.c_double
         L.orc_veff_grad_fd.restype = C.c_double
         L.orc_noise_normal.restype = C.c_double
+        L.orc_bias.restype = C.c_double
+        L.orc_cv_com_distance.restype = C.c_double
         L.orc_noise_bits.restype = C.c_uint64
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -249,3 +251,17 @@ def step_langevin(osys, R, V, dt, n_steps, gamma, temperature, seed=0, step0=0, 
                         C.c_double(KB * temperature), C.c_uint64(seed), C.c_uint64(step0), C.c_int(geom),
                         C.c_int(int(brute)), _p(en))
     return R, V, en
+
+
+def bias(osys, R, group_a, group_b, hills, sigma, height):
+    """MoP bias V(S_e2e) of a path R [N][Q][3].  Returns (V, dV/dR [N][Q][3], (S, s1, sN))."""
+    L = _load()
+    R = np.ascontiguousarray(R, dtype=np.float64)
+    ga = np.ascontiguousarray(group_a, dtype=np.int32)
+    gb = np.ascontiguousarray(group_b, dtype=np.int32)
+    h = np.ascontiguousarray(hills, dtype=np.float64).reshape(-1)
+    g = np.zeros_like(R)
+    out = np.zeros(3)
+    v = L.orc_bias(osys.ref, C.c_int(R.shape[0]), _p(R), _p(ga), C.c_int(len(ga)), _p(gb), C.c_int(len(gb)),
+                   _p(h) if len(h) else None, C.c_int(len(h)), C.c_double(sigma), C.c_double(height), _p(g), _p(out))
+    return float(v), g, tuple(out)

@@ -18,7 +18,7 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
            "mop_set_timing", "mop_get_timing", "mop_probe_fp32", "mop_eval_veff_grad_fd",
-           "mop_step_langevin", "mop_debug_noise_bits"]
+           "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias"]
 
 
 class MopError(RuntimeError):
@@ -81,6 +81,12 @@ def load(build_if_missing=True):
     L.mop_step_langevin.restype = C.c_int
     L.mop_debug_noise_bits.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p]
     L.mop_debug_noise_bits.restype = C.c_int
+    L.mop_set_bias.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int]
+    L.mop_set_bias.restype = C.c_int
+    L.mop_add_hill.argtypes = [C.c_void_p, C.c_double]
+    L.mop_add_hill.restype = C.c_int
+    L.mop_get_bias.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_void_p, C.c_int, C.POINTER(C.c_int)]
+    L.mop_get_bias.restype = C.c_int
     L.mop_probe_fp32.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
@@ -230,6 +236,22 @@ class Mop:
         assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
         self._check(self.L.mop_step_langevin(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps), float(gamma),
                                              float(temperature), int(seed), int(step0)))
+
+    def mop_set_bias(self, group_a, group_b, sigma, height, pace=0):
+        """MoP bias on S_e2e = s(R^N) - s(R^1), s = COM distance of the two groups.  Empty groups switch it off."""
+        ga, gb = _np(group_a, np.int32), _np(group_b, np.int32)
+        self._check(self.L.mop_set_bias(self.ctx, ga.ctypes.data_as(C.c_void_p), len(ga), gb.ctypes.data_as(C.c_void_p),
+                                        len(gb), float(sigma), float(height), int(pace)))
+
+    def mop_add_hill(self, s_center):
+        self._check(self.L.mop_add_hill(self.ctx, float(s_center)))
+
+    def mop_get_bias(self):
+        out = (C.c_double * 8)()
+        n = C.c_int(0)
+        hills = np.zeros(65536)
+        self._check(self.L.mop_get_bias(self.ctx, out, hills.ctypes.data_as(C.c_void_p), len(hills), C.byref(n)))
+        return dict(S=out[0], s1=out[1], sN=out[2], V=out[3], dVdS=out[4], n_hills=int(out[5]), hills=hills[:n.value].copy())
 
     def mop_debug_noise_bits(self, seed, step, n):
         out = np.empty(n, np.uint64)

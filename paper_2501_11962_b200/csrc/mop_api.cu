@@ -9,6 +9,7 @@
 #include <string>
 #include <vector>
 
+#include "mop_bias.cuh"
 #include "mop_bonded.cuh"
 #include "mop_common.cuh"
 #include "mop_grid.cuh"
@@ -66,6 +67,13 @@ struct mop_ctx {
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
+    // metadynamics-of-paths bias (mop_set_bias)
+    bool bias_on = false;
+    int bias_na = 0, bias_nb = 0, bias_pace = 0;
+    long long bias_steps = 0;
+    double bias_sigma = 0, bias_w = 0;
+    int *d_bias_ga = 0, *d_bias_gb = 0, *d_bias_nh = 0;
+    double *d_bias_hills = 0, *d_bias_com = 0, *d_bias_state = 0;
     // finite-difference Hessian mode (mop_eval_veff_grad_fd): [nf][Q][3] buffers in original atom order
     float *d_fdR = 0, *d_fdEta = 0, *d_fdF = 0, *d_fdFp = 0, *d_fdFm = 0;
     // stage timing (mop_set_timing): a ring of event sets, one per evaluation
@@ -137,7 +145,8 @@ static void free_all(mop_ctx *c) {
                     c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
                     c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
                     c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg,       c->d_Rh,
-                    c->d_Gh,      c->d_fdR,      c->d_fdEta,     c->d_fdF,       c->d_fdFp,     c->d_fdFm};
+                    c->d_Gh,      c->d_fdR,      c->d_fdEta,     c->d_fdF,       c->d_fdFp,     c->d_fdFm,
+                    c->d_bias_ga, c->d_bias_gb,  c->d_bias_nh,   c->d_bias_hills, c->d_bias_com, c->d_bias_state};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (c->h_energy) cudaFreeHost(c->h_energy);
@@ -571,7 +580,20 @@ static mop_status read_back(mop_ctx *c) {
     return MOP_OK;
 }
 
-static mop_status eval_async(mop_ctx *c, const float *R, float *grad) {
+// adds dV_bias/dR to grad on beads 1 and N (and deposits a hill at the current S_e2e first when asked to)
+static void bias_launch(mop_ctx *c, const float *R, float *grad, bool deposit) {
+    BiasArgs b;
+    b.Q = c->Q, b.N = c->N, b.na = c->bias_na, b.nb = c->bias_nb;
+    b.ga = c->d_bias_ga, b.gb = c->d_bias_gb, b.mass = c->d_mass;
+    for (int d = 0; d < 3; d++) b.box[d] = c->g.box[d];
+    b.sigma = c->bias_sigma, b.w = c->bias_w;
+    b.hills = c->d_bias_hills, b.n_hills = c->d_bias_nh, b.com = c->d_bias_com, b.state = c->d_bias_state;
+    LAUNCH(c, k_bias_com, dim3(2, 2), 256, 0, b, R);
+    LAUNCH(c, k_bias_cv, 1, 32, 0, b, deposit ? 1 : 0);
+    if (grad) LAUNCH(c, k_bias_apply, dim3(cdiv(b.na + b.nb, 256), 2), 256, 0, b, grad);
+}
+
+static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false) {
     const int nb = c->nf;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
@@ -591,6 +613,7 @@ static mop_status eval_async(mop_ctx *c, const float *R, float *grad) {
         LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->d_slot_of, c->d_F4, c->d_et,
                c->d_H4, c->d_Ki, grad);
     t_mark(c, 8);
+    if (c->bias_on && c->N > 1) bias_launch(c, R, grad, deposit);
     CK(c, cudaGetLastError());
     return MOP_OK;
 }
@@ -715,7 +738,8 @@ extern "C" mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt
     for (int it = 0; it < n_steps; it++) {
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (double *)nullptr);
-        if ((s = eval_async(c, R_dev, c->d_G))) return s;
+        c->bias_steps += 1;
+        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0))) return s;
         const bool last = it == n_steps - 1;
         if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
@@ -743,7 +767,8 @@ extern "C" mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, 
     for (int it = 0; it < n_steps; it++) {
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (double *)nullptr);
-        if ((s = eval_async(c, R_dev, c->d_G))) return s;
+        c->bias_steps += 1;
+        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0))) return s;
         const bool last = it == n_steps - 1;
         if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
@@ -769,6 +794,74 @@ extern "C" mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, 
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
     cudaFree(d);
     CK(c, e);
+    return MOP_OK;
+}
+
+// ---- metadynamics of paths: Gaussian bias on the end-to-end CV
+extern "C" mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, const int *group_b, int n_b, double sigma,
+                                   double height, int pace) {
+    PRECHECK(c);
+    CK(c, cudaStreamSynchronize(c->st));
+    c->bias_on = false;
+    c->bias_steps = 0;
+    if (n_a == 0 && n_b == 0) return MOP_OK;   // bias switched off
+    if (n_a < 1 || n_b < 1 || !group_a || !group_b) FAIL(c, MOP_ERR_INVALID_ARG, "mop_set_bias: both groups need atoms");
+    if (!(sigma > 0.0) || !std::isfinite(height) || pace < 0) FAIL(c, MOP_ERR_INVALID_ARG, "need sigma > 0, finite height, pace >= 0");
+    if (c->N < 2) FAIL(c, MOP_ERR_INVALID_ARG, "the end-to-end CV needs n_beads >= 2");
+    for (int k = 0; k < n_a; k++)
+        if (group_a[k] < 0 || group_a[k] >= c->Q) FAIL(c, MOP_ERR_INVALID_ARG, "group_a[%d] out of range", k);
+    for (int k = 0; k < n_b; k++)
+        if (group_b[k] < 0 || group_b[k] >= c->Q) FAIL(c, MOP_ERR_INVALID_ARG, "group_b[%d] out of range", k);
+    CK(c, dalloc(&c->d_bias_ga, (size_t)n_a));
+    CK(c, dalloc(&c->d_bias_gb, (size_t)n_b));
+    if (!c->d_bias_hills) {
+        CK(c, dalloc(&c->d_bias_hills, (size_t)MOP_MAX_HILLS));
+        CK(c, dalloc(&c->d_bias_nh, 1));
+        CK(c, dalloc(&c->d_bias_com, 16));
+        CK(c, dalloc(&c->d_bias_state, 16));
+    }
+    CK(c, cudaMemcpyAsync(c->d_bias_ga, group_a, (size_t)n_a * 4, cudaMemcpyHostToDevice, c->st));
+    CK(c, cudaMemcpyAsync(c->d_bias_gb, group_b, (size_t)n_b * 4, cudaMemcpyHostToDevice, c->st));
+    CK(c, cudaMemsetAsync(c->d_bias_nh, 0, sizeof(int), c->st));
+    CK(c, cudaMemsetAsync(c->d_bias_state, 0, 16 * sizeof(double), c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    c->bias_na = n_a, c->bias_nb = n_b, c->bias_sigma = sigma, c->bias_w = height, c->bias_pace = pace;
+    c->bias_on = true;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_add_hill(mop_ctx *c, double s_center) {
+    PRECHECK(c);
+    if (!c->bias_on) FAIL(c, MOP_ERR_INVALID_ARG, "mop_add_hill: no bias set");
+    int nh = 0;
+    CK(c, cudaMemcpyAsync(&nh, c->d_bias_nh, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    if (nh >= MOP_MAX_HILLS) FAIL(c, MOP_ERR_OOM, "hill table full (%d)", MOP_MAX_HILLS);
+    CK(c, cudaMemcpyAsync(c->d_bias_hills + nh, &s_center, sizeof(double), cudaMemcpyHostToDevice, c->st));
+    nh += 1;
+    CK(c, cudaMemcpyAsync(c->d_bias_nh, &nh, sizeof(int), cudaMemcpyHostToDevice, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_get_bias(mop_ctx *c, double out[8], double *hills_host, int cap, int *n_hills) {
+    PRECHECK(c);
+    if (!out) FAIL(c, MOP_ERR_INVALID_ARG, "out is NULL");
+    for (int k = 0; k < 8; k++) out[k] = 0.0;
+    if (n_hills) *n_hills = 0;
+    if (!c->bias_on) return MOP_OK;
+    double st[16];
+    int nh = 0;
+    CK(c, cudaMemcpyAsync(st, c->d_bias_state, sizeof st, cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaMemcpyAsync(&nh, c->d_bias_nh, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    for (int k = 0; k < 5; k++) out[k] = st[k];
+    out[5] = (double)nh;
+    if (n_hills) *n_hills = nh;
+    if (hills_host && cap > 0 && nh > 0) {
+        CK(c, cudaMemcpyAsync(hills_host, c->d_bias_hills, (size_t)std::min(cap, nh) * 8, cudaMemcpyDeviceToHost, c->st));
+        CK(c, cudaStreamSynchronize(c->st));
+    }
     return MOP_OK;
 }
 

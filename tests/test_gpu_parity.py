@@ -314,6 +314,56 @@ def test_nvt_temperature_stays_at_target(B, oracle):
     m.close()
 
 
+# --------------------------------------------------------------------------- NEXT-3: the MoP bias on S_e2e
+def test_mop_bias_matches_oracle(B, oracle):
+    """CV, V(S) and the bias gradient on beads 1 and N against the oracle (same FP32 path, explicit hills)."""
+    s, o, R = case(oracle, "chain")
+    ga, gb = np.arange(0, 10), np.arange(10, 19)          # the chain against the three waters: both whole
+    m = B.Mop(s, s.n_beads)
+    v0, g0 = m.mop_eval_veff_grad(R)
+    m.mop_set_bias(ga, gb, 0.002, 3.0)
+    Rd = R.astype(np.float64)
+    _, _, (S_ref, s1_ref, sN_ref) = oracle.bias(o, Rd, ga, gb, [], 0.002, 3.0)
+    hills = [S_ref + 0.001, S_ref - 0.003, S_ref + 0.0004]
+    for h in hills:
+        m.mop_add_hill(h)
+    v1, g1 = m.mop_eval_veff_grad(R)
+    vb_ref, gb_ref, _ = oracle.bias(o, Rd, ga, gb, hills, 0.002, 3.0)
+    st = m.mop_get_bias()
+    assert v1 == pytest.approx(v0, rel=1e-7)                                  # veff_out is eq. (3) without V(S)
+    assert st["n_hills"] == 3 and np.array_equal(st["hills"], np.asarray(hills))
+    assert abs(st["s1"] - s1_ref) <= 1e-12 and abs(st["sN"] - sN_ref) <= 1e-12 and abs(st["S"] - S_ref) <= 1e-12
+    assert st["V"] == pytest.approx(vb_ref, rel=1e-10)
+    dg = (g1 - g0).cpu().numpy().astype(np.float64)
+    assert np.abs(dg[1:-1]).max() <= 1e-6 * np.abs(gb_ref).max()             # interior beads: float-atomic noise only
+    scale = np.abs(gb_ref).max()
+    assert np.abs(dg[0] - gb_ref[0]).max() <= 2e-3 * scale and np.abs(dg[-1] - gb_ref[-1]).max() <= 2e-3 * scale
+    #   (g1 - g0 is a difference of two FP32 gradients of size ~|G|; the bias part itself is exact to FP32 rounding)
+    m.mop_set_bias([], [], 1.0, 0.0)
+    v2, g2 = m.mop_eval_veff_grad(R)
+    assert H.rms_rel(g2.cpu().numpy(), g0.cpu().numpy()) <= 1e-5
+    m.close()
+
+
+def test_mop_hills_are_deposited_every_pace_steps(B, oracle):
+    import torch
+    s, o, R = case(oracle, "c1")
+    m = B.Mop(s, s.n_beads)
+    m.mop_set_bias(np.arange(0, 40), np.arange(200, 260), 0.01, 1.0, pace=3)
+    Rg = torch.tensor(R, device="cuda")
+    Vg = torch.zeros_like(Rg)
+    m.mop_step(Rg, Vg, 0.001, 7)
+    assert m.mop_get_bias()["n_hills"] == 2
+    m.mop_step_langevin(Rg, Vg, 0.001, 2, 50.0, s.temperature, seed=3, step0=7)   # step 9 deposits the third hill
+    st = m.mop_get_bias()
+    assert st["n_hills"] == 3 and st["hills"][2] == st["S"]
+    _, _, (S_ref, _, _) = oracle.bias(o, Rg.cpu().numpy().astype(np.float64), np.arange(0, 40), np.arange(200, 260), [], 0.01, 1.0)
+    assert abs(st["S"] - S_ref) <= 1e-9
+    with pytest.raises(B.MopError):
+        m.mop_set_bias([0], [s.n_atoms], 0.01, 1.0)
+    m.close()
+
+
 # --------------------------------------------------------------------------- degenerate inputs and errors
 def test_edge_cases(B, oracle):
     # two atoms, one pair; then out of range

@@ -412,6 +412,45 @@ def test_P14_nvt_temperature_of_an_interacting_path(oracle):
     assert abs(t_kin.mean() / T - 1.0) < 0.04
 
 
+# ---------------------------------------------------------------- P15 MoP bias (NEXT-3)
+def test_P15_bias_closed_forms_and_gradient(oracle):
+    """(i) two single-atom groups: s is their distance, S_e2e the difference between last and first bead, one hill
+    at S gives V = w and zero force; (ii) dV/dR against central differences of V; (iii) the bias force on each end
+    bead sums to zero (translation invariance) and vanishes on interior beads."""
+    s = H.lj_cluster(32, masses=np.linspace(5, 40, 32))
+    o = oracle.OracleSystem(s)
+    rng = np.random.default_rng(6)
+    R = s.R1[None] + rng.normal(0, 0.02, (4, 32, 3))
+    box = np.asarray(s.box, float)
+    mi = lambda d: d - box * np.round(d / box)            # minimum image of the COM difference
+    d1 = np.linalg.norm(mi(R[0, 3] - R[0, 17]))
+    dN = np.linalg.norm(mi(R[3, 3] - R[3, 17]))
+    v, g, (S, s1, sN) = oracle.bias(o, R, [3], [17], [dN - d1], 0.05, 2.5)
+    assert s1 == pytest.approx(d1, rel=1e-14) and sN == pytest.approx(dN, rel=1e-14) and S == pytest.approx(dN - d1, abs=1e-14)
+    assert v == pytest.approx(2.5, rel=1e-12) and np.abs(g).max() < 1e-9
+    v, g, (S, s1, sN) = oracle.bias(o, R, [3], [17], [S + 0.03], 0.05, 2.5)
+    assert v == pytest.approx(2.5 * np.exp(-0.5 * 0.36), rel=1e-10)
+    ga, gb = np.arange(0, 9), np.arange(20, 32)
+    hills = [0.01, -0.04, 0.08]
+    v, g, (S, s1, sN) = oracle.bias(o, R, ga, gb, hills, 0.05, 2.5)
+    M = s.mass.astype(float)
+    com = lambda X, idx: (M[idx, None] * X[idx]).sum(0) / M[idx].sum()
+    assert s1 == pytest.approx(np.linalg.norm(mi(com(R[0], ga) - com(R[0], gb))), rel=1e-13)
+    assert np.abs(g[1:3]).max() == 0.0 and np.abs(g[0]).max() > 0 and np.abs(g[3]).max() > 0
+    assert np.abs(g[0].sum(0)).max() < 1e-12 * np.abs(g[0]).max() and np.abs(g[3].sum(0)).max() < 1e-12 * np.abs(g[3]).max()
+    e = 1e-6
+    for n, i, a in ((0, 2, 0), (0, 25, 2), (3, 7, 1), (3, 30, 0), (3, 15, 1)):
+        Rp, Rm = R.copy(), R.copy()
+        Rp[n, i, a] += e
+        Rm[n, i, a] -= e
+        fd = (oracle.bias(o, Rp, ga, gb, hills, 0.05, 2.5)[0] - oracle.bias(o, Rm, ga, gb, hills, 0.05, 2.5)[0]) / (2 * e)
+        assert fd == pytest.approx(g[n, i, a], rel=1e-6, abs=1e-9)
+    # periodic images of a whole group do not change s
+    R2 = R.copy()
+    R2[:, gb] += np.asarray(s.box, float) * [1, -2, 0]
+    assert oracle.bias(o, R2, ga, gb, hills, 0.05, 2.5)[0] == pytest.approx(v, rel=1e-10)
+
+
 # ---------------------------------------------------------------- P13 + G8 neighbour sets
 @pytest.mark.parametrize("mk", ["c1", "c2", "tiny", "edge"])
 def test_P13_cell_list_equals_brute_force(oracle, mk):

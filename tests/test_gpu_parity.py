@@ -387,6 +387,31 @@ def test_edge_cases(B, oracle):
     m.close()
 
 
+def test_box_barely_above_twice_the_cutoff(B, oracle):
+    """min(box) = 2.0001 r_c: every cluster pair is listed under several periodic shifts (up to 27 work units per
+    i-cluster); the in-range image of an atom pair is still unique.  Also a rectangular box with one tight side."""
+    for box in ([2.0001] * 3, [2.0001, 3.3, 2.6]):
+        s = H.lj_cluster(64, L=2.0001, r_cut=1.0)
+        if box[1] != box[0]:
+            rng = np.random.default_rng(4)
+            X = rng.uniform(0, 1, (96, 3)) * np.asarray(box)
+            s = H.make_system("rect", box, X, np.full(96, 39.948), rng.normal(0, 0.2, 96), np.zeros(96, int), [0.2],
+                              [0.3], r_cut=1.0, eps_rf=78.0, lj_shift=1, T=120.0)
+        s.n_beads = 3
+        o = oracle.OracleSystem(s)
+        R = W.brownian_path(s, 3, lambda X: oracle.bead(o, X, geom=0, brute=True)["F"], seed=0)
+        m = B.Mop(s, 3)
+        v, g = m.mop_eval_veff_grad(R)
+        for n in range(m.nf):
+            ref = oracle.pairs(o, R[n].astype(np.float64), geom=1, brute=True)
+            got, cnt = m.mop_debug_pairs(n)
+            assert cnt == len(ref) and np.array_equal(got, ref)
+        v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=True)
+        assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+        assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+        m.close()
+
+
 def test_atoms_outside_the_box_and_on_faces(B, oracle):
     """Caller coordinates are never wrapped per bead; atoms far outside [0,L) and exactly on faces."""
     s, o, R = case(oracle, "c1")

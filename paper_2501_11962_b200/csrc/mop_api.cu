@@ -40,7 +40,7 @@ struct mop_ctx {
     // topology (device)
     int nt = 0, n_bonds = 0, n_angles = 0, max_excl = 0;
     float *d_mass = 0, *d_inv_mass = 0, *d_charge = 0, *d_ai = 0, *d_Ki = 0, *d_tabs = 0;
-    float2 *d_tab = 0, *d_tabe = 0, *d_bond_par = 0, *d_angle_par = 0;
+    float2 *d_tab = 0, *d_bond_par = 0, *d_angle_par = 0;
     int *d_type_row = 0, *d_bond_ij = 0, *d_angle_ijk = 0, *d_excl_start = 0, *d_excl_list = 0;
     // per-bead sorted state
     int *d_cell = 0, *d_cell_count = 0, *d_cell_rel = 0, *d_cell_fill = 0, *d_col_count = 0, *d_col_start = 0;
@@ -139,7 +139,7 @@ extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_st
 
 static void free_all(mop_ctx *c) {
     void *ptrs[] = {c->d_mass,    c->d_inv_mass, c->d_charge,    c->d_ai,        c->d_Ki,       c->d_tabs,
-                    c->d_tab,     c->d_tabe, c->d_bond_par, c->d_angle_par, c->d_type_row,  c->d_bond_ij,  c->d_angle_ijk,
+                    c->d_tab,     c->d_bond_par, c->d_angle_par, c->d_type_row,  c->d_bond_ij,  c->d_angle_ijk,
                     c->d_excl_start, c->d_excl_list, c->d_cell,  c->d_cell_count, c->d_cell_rel, c->d_cell_fill,
                     c->d_col_count, c->d_col_start, c->d_tmp,    c->d_perm,      c->d_slot_of,  c->d_typ,
                     c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
@@ -349,7 +349,7 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     // derived host arrays
     std::vector<float> inv_m(Q), ai(Q), Ki(Q), tabs(nt * nt);
     std::vector<int> trow(Q);
-    std::vector<float2> tab(nt * nt), tabe(nt * nt);
+    std::vector<float2> tab(nt * nt);
     for (int i = 0; i < Q; i++) {
         double m = (double)t->mass[i];
         inv_m[i] = (float)(1.0 / m);
@@ -360,7 +360,6 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     const double rc = (double)c->p.r_cut, irc6 = 1.0 / (rc * rc * rc * rc * rc * rc);
     for (int k = 0; k < nt * nt; k++) {
         tab[k] = make_float2(6.0f * t->c6[k], 12.0f * t->c12[k]);
-        tabe[k] = make_float2(t->c6[k], t->c12[k]);
         tabs[k] = c->p.lj_shift ? (float)((double)t->c12[k] * irc6 * irc6 - (double)t->c6[k] * irc6) : 0.0f;
     }
     auto up = [&](auto **dst, const void *src, size_t n, size_t esz) -> cudaError_t {
@@ -376,7 +375,6 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     CK(c, up(&c->d_Ki, Ki.data(), Q, 4));
     CK(c, up(&c->d_type_row, trow.data(), Q, 4));
     CK(c, up(&c->d_tab, tab.data(), (size_t)nt * nt, 8));
-    CK(c, up(&c->d_tabe, tabe.data(), (size_t)nt * nt, 8));
     CK(c, up(&c->d_tabs, tabs.data(), (size_t)nt * nt, 4));
     CK(c, up(&c->d_bond_ij, t->bond_ij, (size_t)2 * t->n_bonds, 4));
     CK(c, up(&c->d_bond_par, t->bond_b0_kb, (size_t)t->n_bonds, 8));
@@ -512,7 +510,7 @@ static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.work = c->d_work + work_slot;
     a.range = range;
-    a.tab = c->d_tab, a.tabe = c->d_tabe, a.tabs = c->d_tabs;
+    a.tab = c->d_tab, a.tabs = c->d_tabs;
     a.energies = c->d_energy;
     for (int d = 0; d < 3; d++) a.box[d] = c->g.box[d];
     return a;

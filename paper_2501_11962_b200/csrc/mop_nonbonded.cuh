@@ -27,7 +27,6 @@ struct NbArgs {
     unsigned *work;     // dynamic work counter (zeroed before the launch)
     int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all
     const float2 *tab;  // [nt*nt] (6 C6, 12 C12)
-    const float2 *tabe; // [nt*nt] (C6, C12) as given (energy: no rounding bias from the prefactors)
     const float *tabs;  // [nt*nt] LJ energy shift C12 rc^-12 - C6 rc^-6 (0 when lj_shift = 0)
     double *energies;   // [0] U_lj, [1] U_coul
     float box[3];

@@ -97,18 +97,18 @@ enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
 //                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
 //   [1024, 2048)           the current chunk of up to 32 list entries, 256 B per warp
 //   [2048, 2048 + 16 KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
-//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), (C6, C12)[nt*nt] as given, energy shift [nt*nt],
+//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), energy shift [nt*nt],
 //   and one flag per type: its LJ row has a non-zero entry
 #define NBP_SM_ENT 1024u
 #define NBP_SM_RING 2048u
 #define NBP_SM_TAB (2048u + 4u * NBP_NST * 1024u)
-__host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 20 + (size_t)nt * 4; }
+__host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 12 + (size_t)nt * 4; }
 
 template <int MODE, int VAR>
 __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, float *__restrict__ sw,
                                          const unsigned sw_addr, const unsigned se_addr, const unsigned sr_addr,
                                          const unsigned tab6, const unsigned off12,
-                                         const float2 *__restrict__ tabe, const float *__restrict__ tabs,
+                                         const float *__restrict__ tabs,
                                          const int *__restrict__ tflag, const int lane) {
     constexpr bool HVP = MODE == NB_HVP, ENERGY = MODE == NB_ENERGY;
     const unsigned boff = (unsigned)un.bead * (unsigned)a.S; // nf * S < 2^31 (checked at create)
@@ -222,7 +222,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 if (ENERGY) { // u_lj = C12 x^6 - C6 x^3 - shift = B/12 - A/6 - shift;  u_c = ke qi qj (1/r + k_rf r^2 - c_rf)
                     f2 ue = f2_mul(qq, f2_add(f2_fma(r2v[p], f2_bc(a.krf), rinv), f2_bc(-a.crf)));
                     if (!nolj) {
-                        const f2 sh = f2_pack(mop_lds_f(ta + 4u * off12), mop_lds_f(tb + 4u * off12));
+                        const f2 sh = f2_pack(mop_lds_f(ta + 2u * off12), mop_lds_f(tb + 2u * off12));
                         const f2 ul = f2_fma(B, f2_bc(1.0f / 12.0f), f2_fma(A, f2_bc(-1.0f / 6.0f), f2_mul(sh, f2_bc(-1.0f))));
                         float la, lb;
                         f2_unpack(ul, la, lb);
@@ -367,13 +367,11 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
     float *sw = reinterpret_cast<float *>(sb) + w * 64;
     const int n2 = a.nt * a.nt;
     float *t6 = reinterpret_cast<float *>(sb + NBP_SM_TAB), *t12 = t6 + n2;
-    float2 *tabe = reinterpret_cast<float2 *>(t12 + n2);
-    float *tabs = reinterpret_cast<float *>(tabe + n2);
+    float *tabs = t12 + n2;
     int *tflag = reinterpret_cast<int *>(tabs + n2);   // [nt]: 1 iff the type's LJ row has a non-zero entry
     for (int t = threadIdx.x; t < n2; t += blockDim.x) {
         const float2 c = a.tab[t];
         t6[t] = c.x, t12[t] = c.y;
-        tabe[t] = a.tabe[t];
         tabs[t] = a.tabs[t];
     }
     for (int t = threadIdx.x; t < a.nt; t += blockDim.x) {
@@ -400,6 +398,6 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
         un.bead = (int)u0.x, un.ci = (int)u0.y, un.shift = (int)u0.z, un.start = u0.w;
         un.count = u1.x, un.excl_base = u1.y;
         if (un.count == 0) continue;
-        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabe, tabs, tflag, lane);
+        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabs, tflag, lane);
     }
 }

@@ -90,13 +90,13 @@ __device__ __forceinline__ void mop_cp_wait() {
 
 enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
        NBP_OCC6 = 4 };  // ask for 6 resident CTAs per SM (register cap 80)
-#define NBP_NST 4       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1)
+#define NBP_NST 2       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1; 2 measured best of 2, 3, 4, 6)
 
 // Shared memory of one CTA (4 warps), bytes:
 //   [0, 1024)              i-atom staging, 256 B per warp: for p = 0..3 at float offset 16 p
 //                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
 //   [1024, 2048)           the current chunk of up to 32 list entries, 256 B per warp
-//   [2048, 2048 + 16 KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
+//   [2048, 2048 + 4 NBP_NST KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
 //   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), energy shift [nt*nt],
 //   and one flag per type: its LJ row has a non-zero entry
 #define NBP_SM_ENT 1024u

@@ -432,6 +432,42 @@ def test_atoms_outside_the_box_and_on_faces(B, oracle):
     m.close()
 
 
+def test_host_buffer_entry_point_matches_device_one(B, oracle):
+    """mop_eval_veff_grad_host (pinned host buffers in and out: the end-to-end form bench.py times) gives the device
+    entry point's numbers."""
+    import torch
+    s, o, R = case(oracle, "c2")
+    m = B.Mop(s, s.n_beads)
+    v, g = m.mop_eval_veff_grad(R)
+    Rh = torch.as_tensor(R).pin_memory()
+    Gh = torch.empty_like(Rh).pin_memory()
+    vh = m.mop_eval_veff_grad_host(Rh, Gh)
+    assert abs(vh - v) <= 1e-7 * abs(v)
+    assert H.rms_rel(Gh.numpy(), g.cpu().numpy()) <= 1e-5
+    m.close()
+
+
+def test_argument_errors_of_the_added_entry_points(B):
+    import torch
+    s = W.config1(n_beads=1)
+    m = B.Mop(s, 1)
+    with pytest.raises(B.MopError) as e:          # the end-to-end CV needs two beads
+        m.mop_set_bias([0], [1], 0.01, 1.0)
+    assert e.value.status == 1
+    R = torch.tensor(np.float32(s.R1)[None], device="cuda")
+    V = torch.zeros_like(R)
+    with pytest.raises(B.MopError):
+        m.mop_step_langevin(R, V, 0.001, 1, -1.0, 300.0)
+    with pytest.raises(B.MopError):
+        m.mop_eval_veff_grad_fd(R, 0.0)
+    with pytest.raises(B.MopError):
+        m.mop_add_hill(0.0)                       # no bias set
+    v, g = m.mop_eval_veff_grad_fd(R, 0.01)       # N = 1: plain -F
+    v2, g2 = m.mop_eval_veff_grad(R)
+    assert v == pytest.approx(v2, rel=1e-7) and H.rms_rel(g.cpu().numpy(), g2.cpu().numpy()) <= 1e-5
+    m.close()
+
+
 def test_error_codes(B):
     s = W.config1(n_beads=2)
     s.box = np.asarray([1.9, 2.88, 2.88], np.float32)

@@ -125,7 +125,7 @@ const char *mop_last_error(const mop_ctx *c);
 /* Synchronises.  out[0]=V_eff, [1]=U(R^1), [2]=E_spring, [3]=U_lj(R^1), [4]=U_coul(R^1), [5]=U_bond(R^1),
  * [6]=U_angle(R^1), [7]=kinetic energy after the last mop_step, [8]=pair-list rebuilds so far,
  * [9]=cluster-pair entries in the current list, [10]=list units, [11]=exclusion masks,
- * [12]=pair slots evaluated per nonbonded pass (entries * 8 * 32), [13]=kernel launches so far,
+ * [12]=pair slots the list admits per nonbonded pass (sum over entries of popcount(i-atom mask) * 32), [13]=kernel launches so far,
  * [14],[15] reserved. */
 mop_status mop_get_stats(mop_ctx *c, double out[16]);
 

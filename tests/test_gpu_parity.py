@@ -412,6 +412,39 @@ def test_box_barely_above_twice_the_cutoff(B, oracle):
         m.close()
 
 
+def test_maximum_number_of_types(B, oracle):
+    """n_types = 64 (the header's maximum; 59 KB of dynamic shared memory for the LJ tables) with several all-zero
+    LJ rows (the reaction-field-only body) and charges; 65 types are rejected."""
+    rng = np.random.default_rng(12)
+    n, nt = 300, 64
+    box = [2.7, 2.9, 3.1]
+    g = np.stack(np.meshgrid(np.arange(6), np.arange(7), np.arange(8), indexing="ij"), -1).reshape(-1, 3)[:n]
+    X = (g + 0.5) * (np.asarray(box) / [6, 7, 8]) + rng.normal(0, 0.02, (n, 3))
+    sig = rng.uniform(0.25, 0.36, nt)
+    eps = rng.uniform(0.2, 1.0, nt)
+    eps[::5] = 0.0                                   # every fifth type has no LJ at all
+    typ = rng.integers(0, nt, n)
+    q = rng.normal(0, 0.3, n)
+    s = H.make_system("types64", box, X, rng.uniform(5, 40, n), q - q.mean(), typ, list(sig), list(eps), r_cut=1.0,
+                      eps_rf=78.0, lj_shift=1, T=200.0)
+    s.n_beads = 3
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 3, lambda Y: oracle.bead(o, Y, geom=0, brute=True)["F"], seed=0)
+    m = B.Mop(s, 3)
+    v, g_ = m.mop_eval_veff_grad(R)
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=True)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g_.cpu().numpy(), g_ref) <= TOL_RMS
+    ref = oracle.pairs(o, R[0].astype(np.float64), geom=1, brute=True)
+    got, cnt = m.mop_debug_pairs(0)
+    assert cnt == len(ref) and np.array_equal(got, ref)
+    m.close()
+    s2 = H.make_system("types65", box, X, rng.uniform(5, 40, n), q - q.mean(), typ, list(sig) + [0.3], list(eps) + [0.5])
+    with pytest.raises(B.MopError) as e:
+        B.Mop(s2, 2)
+    assert e.value.status == 1
+
+
 def test_atoms_outside_the_box_and_on_faces(B, oracle):
     """Caller coordinates are never wrapped per bead; atoms far outside [0,L) and exactly on faces."""
     s, o, R = case(oracle, "c1")

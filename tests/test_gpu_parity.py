@@ -412,6 +412,24 @@ def test_box_barely_above_twice_the_cutoff(B, oracle):
         m.close()
 
 
+def test_many_beads(B, oracle):
+    """N = 130 beads of the 512-atom LJ system (more beads than the largest sweep point): V_eff, gradient, and the
+    neighbour sets of the first and last force bead."""
+    s = W.config1(n_beads=130)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 130, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    m = B.Mop(s, 130)
+    v, g = m.mop_eval_veff_grad(R)
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=False)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    for n in (0, m.nf - 1):
+        ref = oracle.pairs(o, R[n].astype(np.float64), geom=1, brute=True)
+        got, cnt = m.mop_debug_pairs(n)
+        assert cnt == len(ref) and np.array_equal(got, ref)
+    m.close()
+
+
 def test_maximum_number_of_types(B, oracle):
     """n_types = 64 (the header's maximum; 59 KB of dynamic shared memory for the LJ tables) with several all-zero
     LJ rows (the reaction-field-only body) and charges; 65 types are rejected."""

@@ -54,10 +54,13 @@ typedef struct {
     int n_beads;      /* N >= 1 */
     float box[3];     /* rectangular periodic box (nm) */
     float r_cut;      /* nonbonded cutoff (nm), > 0 */
-    float r_buf;      /* list margin (nm), >= 0: the cluster-pair list is built with r_cut + r_buf.  This build rebuilds
-                         the list in EVERY evaluation (bench.py times it that way), so 0 is the efficient value; reuse
-                         of a buffered list across evaluations is not implemented.  Results never depend on r_buf:
-                         the r_cut test is applied per atom pair in the pair kernels */
+    float r_buf;      /* Verlet buffer (nm), >= 0.  0: the pair list is rebuilt in every evaluation and the neighbour
+                         sets follow the bit-exact predicate of DESIGN.md (reading G8).  > 0: the list is built with
+                         r_cut + r_buf and kept while no atom of a force bead has moved farther than r_buf/2 from
+                         where it was at the build; a reusing evaluation refreshes the sorted coordinates in the
+                         periodic image of that build (wrap(R_ref) + (R - R_ref): the same pairs to FP32 rounding
+                         of r^2, not bit for bit) and reads one flag on the host, which synchronises the stream.
+                         Results never depend on the list: the r_cut test is applied per atom pair */
     float eps_rf;     /* reaction-field dielectric; <= 0 means infinity (k_rf = 1/(2 r_cut^3)) */
     int lj_shift;     /* 1: potential-shift the LJ energy so that U_LJ(r_cut) = 0 (forces unchanged) */
     double dt_path;   /* path spacing Delta t (ps): enters K_i and L^n only */
@@ -126,7 +129,7 @@ const char *mop_last_error(const mop_ctx *c);
  * [6]=U_angle(R^1), [7]=kinetic energy after the last mop_step, [8]=pair-list rebuilds so far,
  * [9]=cluster-pair entries in the current list, [10]=list units, [11]=exclusion masks,
  * [12]=pair slots the list admits per nonbonded pass (sum over entries of popcount(i-atom mask) * 32), [13]=kernel launches so far,
- * [14],[15] reserved. */
+ * [14]=evaluations that reused a buffered list (r_buf > 0), [15] reserved. */
 mop_status mop_get_stats(mop_ctx *c, double out[16]);
 
 /* Stage timing with CUDA events on the context stream (the stream the kernels are launched on).  on != 0: every

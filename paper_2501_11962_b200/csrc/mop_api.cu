@@ -67,6 +67,11 @@ struct mop_ctx {
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
+    // reuse of a buffered pair list (r_buf > 0)
+    bool list_valid = false;
+    float *d_Rref = 0;      // [nf][Q][3] caller coordinates at the last build
+    int *d_moved = 0, *h_moved = 0;
+    double n_reuses = 0;
     // metadynamics-of-paths bias (mop_set_bias)
     bool bias_on = false;
     int bias_na = 0, bias_nb = 0, bias_pace = 0;
@@ -146,12 +151,14 @@ static void free_all(mop_ctx *c) {
                     c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
                     c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg,       c->d_Rh,
                     c->d_Gh,      c->d_fdR,      c->d_fdEta,     c->d_fdF,       c->d_fdFp,     c->d_fdFm,
+                    c->d_Rref,    c->d_moved,
                     c->d_bias_ga, c->d_bias_gb,  c->d_bias_nh,   c->d_bias_hills, c->d_bias_com, c->d_bias_state};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (c->h_energy) cudaFreeHost(c->h_energy);
     if (c->h_ctr) cudaFreeHost(c->h_ctr);
     if (c->h_slots) cudaFreeHost(c->h_slots);
+    if (c->h_moved) cudaFreeHost(c->h_moved);
     if (c->ev_made)
         for (auto &set : c->ev)
             for (cudaEvent_t e : set) cudaEventDestroy(e);
@@ -430,6 +437,7 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     }
     CK(c, cudaStreamSynchronize(c->st));
     c->has_topology = true;
+    c->list_valid = false;
     return MOP_OK;
 }
 
@@ -591,12 +599,44 @@ static void bias_launch(mop_ctx *c, const float *R, float *grad, bool deposit) {
     if (grad) LAUNCH(c, k_bias_apply, dim3(cdiv(b.na + b.nb, 256), 2), 256, 0, b, grad);
 }
 
+// S0 + S1 of an evaluation.  r_buf = 0: always a fresh build.  r_buf > 0: the list of the last build is kept while no
+// atom has moved farther than r_buf / 2 from where it was then (k_refresh re-fills the sorted coordinates in the
+// image of that build; the host reads one flag, which synchronises the stream).
+static mop_status list_for(mop_ctx *c, const float *R, int nb) {
+    if (c->p.r_buf > 0.f && c->list_valid) {
+        if (!c->d_moved) {
+            CK(c, dalloc(&c->d_moved, 1));
+            CK(c, cudaMallocHost((void **)&c->h_moved, sizeof(int)));
+        }
+        CK(c, cudaMemsetAsync(c->d_moved, 0, sizeof(int), c->st));
+        const float hb = 0.5f * c->p.r_buf;
+        LAUNCH(c, k_refresh, dim3(cdiv(c->Q, 256), nb), 256, 0, R, c->d_Rref, c->g, hb * hb, c->d_slot_of, c->d_xq,
+               c->d_moved);
+        CK(c, cudaMemcpyAsync(c->h_moved, c->d_moved, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+        CK(c, cudaStreamSynchronize(c->st));
+        if (*c->h_moved == 0) {
+            c->n_reuses += 1;
+            t_mark(c, 1), t_mark(c, 2);
+            return MOP_OK;
+        }
+    }
+    mop_status s = build_list(c, R, nb, true);
+    if (s) return s;
+    if (c->p.r_buf > 0.f) {
+        const size_t bytes = (size_t)nb * c->Q * 3 * sizeof(float);
+        if (!c->d_Rref) CK(c, dalloc(&c->d_Rref, (size_t)c->nf * c->Q * 3));
+        CK(c, cudaMemcpyAsync(c->d_Rref, R, bytes, cudaMemcpyDeviceToDevice, c->st));
+        c->list_valid = true;
+    }
+    return MOP_OK;
+}
+
 static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false) {
     const int nb = c->nf;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
     t_mark(c, 0);
-    mop_status s = build_list(c, R, nb, true);
+    mop_status s = list_for(c, R, nb);
     if (s) return s;
     if ((s = pass_force(c, R, nb, true))) return s;
     if (c->N > 1) {
@@ -656,6 +696,7 @@ extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, doub
     const dim3 gq(cdiv(c->Q, 256), nb);
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    c->list_valid = false;   // the displaced configurations below overwrite the list
     mop_status s = build_list(c, R_dev, nb);
     if (s) return s;
     if ((s = pass_force(c, R_dev, nb))) return s;
@@ -880,7 +921,8 @@ extern "C" mop_status mop_get_stats(mop_ctx *c, double out[16]) {
     out[11] = (double)c->h_ctr->n_masks;
     out[12] = (double)(*c->h_slots) * 32.0;
     out[13] = c->n_launches;
-    out[14] = out[15] = 0.0;
+    out[14] = c->n_reuses;
+    out[15] = 0.0;
     return MOP_OK;
 }
 
@@ -947,6 +989,7 @@ extern "C" mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float 
     if (Hs_dev && !s_dev) FAIL(c, MOP_ERR_INVALID_ARG, "Hs_dev needs s_dev");
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    c->list_valid = false;
     mop_status s = build_list(c, R_dev, 1);
     if (s) return s;
     if ((s = pass_force(c, R_dev, 1))) return s;

@@ -174,3 +174,23 @@ __global__ void __launch_bounds__(128) k_bbox(MopGrid g, const int *__restrict__
         jhi[oj] = make_float4(hi[0], hi[1], hi[2], 0.0f);
     }
 }
+
+// ---- reuse of a buffered list (r_buf > 0): refresh the sorted coordinates in place -------------------------------
+// Every atom keeps the slot and the periodic image it had when the list was built:
+//   xq[slot] = wrap(R_ref) + (R - R_ref)      (never re-wrapped: the list's unit shifts stay valid)
+// and the flag is raised when some atom has moved farther than r_buf / 2 from R_ref (the list then misses pairs and
+// the caller rebuilds).  One thread per (bead, atom).
+__global__ void __launch_bounds__(256) k_refresh(const float *__restrict__ R, const float *__restrict__ Rref, MopGrid g,
+                                                 float half_buf2, const int *__restrict__ slot_of,
+                                                 float4 *__restrict__ xq, int *__restrict__ flag) {
+    const int n = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.Q) return;
+    const float *r = R + ((size_t)n * g.Q + i) * 3, *f = Rref + ((size_t)n * g.Q + i) * 3;
+    const float dx = r[0] - f[0], dy = r[1] - f[1], dz = r[2] - f[2];
+    if (!(dx * dx + dy * dy + dz * dz <= half_buf2)) *flag = 1;   // also catches NaN
+    float4 *p = xq + (size_t)n * g.S + slot_of[(size_t)n * g.Q + i];
+    p->x = mop_wrap1(f[0], g.box[0], g.inv_box[0]) + dx;
+    p->y = mop_wrap1(f[1], g.box[1], g.inv_box[1]) + dy;
+    p->z = mop_wrap1(f[2], g.box[2], g.inv_box[2]) + dz;
+}

@@ -412,6 +412,36 @@ def test_box_barely_above_twice_the_cutoff(B, oracle):
         m.close()
 
 
+def test_buffered_list_reuse(B, oracle):
+    """r_buf > 0: the list survives displacements below r_buf/2 (stats count the reuses), a larger move rebuilds it, and
+    every evaluation still matches the oracle on the moved coordinates (the r_c test is per atom pair)."""
+    s, o, R = case(oracle, "c2")
+    m = B.Mop(s, s.n_beads, r_buf=0.08)
+    rng = np.random.default_rng(31)
+    Rk = R.copy()
+    for k in range(4):
+        v, g = m.mop_eval_veff_grad(Rk)
+        v_ref, g_ref = oracle.veff_grad(o, Rk.astype(np.float64), geom=1, brute=False)
+        assert abs(v - v_ref) <= TOL_V * abs(v_ref), k
+        assert H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS, k
+        ref = oracle.pairs(o, Rk[0].astype(np.float64), geom=1, brute=True)
+        assert abs(m.mop_debug_pairs(0, cap=0)[1] - len(ref)) <= 2        # same pairs up to FP32 rounding of r^2 at r_c
+        st = m.mop_get_stats()
+        assert (st["rebuilds"], st["reuses"]) == ((1, k) if k < 3 else (2, 2)), (k, st["rebuilds"], st["reuses"])
+        step = 0.008 if k < 2 else 0.06                                   # the third move exceeds r_buf / 2 = 0.04
+        Rk = (Rk + rng.uniform(-1, 1, Rk.shape).astype(np.float32) * np.float32(step / np.sqrt(3))).astype(np.float32)
+    # atoms that cross a box face keep their image: shift everything by 0.03 nm along x twice
+    m2 = B.Mop(s, s.n_beads, r_buf=0.08)
+    for k in range(2):
+        Rs = (R + np.float32([0.03 * k, 0, 0])).astype(np.float32)
+        v, g = m2.mop_eval_veff_grad(Rs)
+        v_ref, g_ref = oracle.veff_grad(o, Rs.astype(np.float64), geom=1, brute=False)
+        assert abs(v - v_ref) <= TOL_V * abs(v_ref) and H.rms_rel(g.cpu().numpy(), g_ref) <= TOL_RMS
+    assert m2.mop_get_stats()["reuses"] == 1
+    m.close()
+    m2.close()
+
+
 def test_many_beads(B, oracle):
     """N = 130 beads of the 512-atom LJ system (more beads than the largest sweep point): V_eff, gradient, and the
     neighbour sets of the first and last force bead."""

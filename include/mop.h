@@ -43,9 +43,11 @@ typedef enum {
     MOP_ERR_INVALID_ARG = 1,   /* bad size, pointer, index, non-positive mass, asymmetric exclusions */
     MOP_ERR_NO_TOPOLOGY = 2,   /* eval/step before mop_set_topology */
     MOP_ERR_BOX_TOO_SMALL = 3, /* min(box) < 2 (r_cut + r_buf): the in-range periodic image would not be unique */
-    MOP_ERR_OOM = 4,           /* device allocation failed or a pair-list buffer overflowed */
+    MOP_ERR_OOM = 4,           /* device allocation failed, or a pair-list buffer overflowed (not sticky: the buffers
+                                  are regrown from the builder's counts and the call can be repeated) */
     MOP_ERR_CUDA = 5,          /* any CUDA runtime error (sticky), or no device */
-    MOP_ERR_NONFINITE = 6      /* V_eff came out NaN/Inf (overlapping atoms) */
+    MOP_ERR_NONFINITE = 6      /* V_eff came out NaN/Inf (overlapping atoms), or an input coordinate is NaN/Inf or
+                                  farther than ~1e6 box lengths from the box (sticky) */
 } mop_status;
 
 /* Problem statement of PAPER.md:36-52: Q atoms, N beads at path spacing dt, friction nu.  Copied at create. */
@@ -102,7 +104,8 @@ mop_status mop_set_topology(mop_ctx *c, const mop_topology *t);
  *   grad_dev DEVICE [N][Q][3] float, dV_eff/dR^n_i in kJ/mol/nm, caller-allocated; NULL: not written.
  * Passes: S0 bin+sort, S1 pair list, S2 nonbonded force, S3 bonded force,
  * S4 eta + spring energy, S5 nonbonded H.eta, S6 bonded H.eta, S7 assembly.
- * Errors: NO_TOPOLOGY, INVALID_ARG, OOM (list overflow, reported at a synchronising call), CUDA, NONFINITE. */
+ * Errors: NO_TOPOLOGY, INVALID_ARG, OOM (list overflow: flagged on the device by any build, reported at the next
+ * synchronising call, after which the regrown buffers let the call be repeated), CUDA, NONFINITE. */
 mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double *veff_out, float *grad_dev);
 
 /* The same evaluation with HOST buffers (the end-to-end form): copies R_host [N][Q][3] to the device on the
@@ -114,7 +117,7 @@ mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff
 /* n_steps velocity-Verlet steps of eq. (4) with F_eff = -grad V_eff and masses m_i, step dt_pmd (ps):
  *   v += dt/2 F_eff/m ; R += dt v ; F_eff(R) ; v += dt/2 F_eff/m.
  * R_dev, V_dev DEVICE [N][Q][3] float, updated in place.  The gradient at the incoming R is evaluated at the
- * start of every call (n_steps + 1 evaluations per call).  Asynchronous. */
+ * start of every call (n_steps + 1 evaluations per call; mop_step_continue skips it).  Asynchronous. */
 mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps);
 
 /* NULL-safe; frees all library-owned memory. */
@@ -128,7 +131,7 @@ const char *mop_last_error(const mop_ctx *c);
 /* Synchronises.  out[0]=V_eff, [1]=U(R^1), [2]=E_spring, [3]=U_lj(R^1), [4]=U_coul(R^1), [5]=U_bond(R^1),
  * [6]=U_angle(R^1), [7]=kinetic energy after the last mop_step, [8]=pair-list rebuilds so far,
  * [9]=cluster-pair entries in the current list, [10]=list units, [11]=exclusion masks,
- * [12]=pair slots the list admits per nonbonded pass (sum over entries of popcount(i-atom mask) * 32), [13]=kernel launches so far,
+ * [12]=pair slots the list admits per nonbonded pass (sum over entries of popcount(row-pair pattern) * 16), [13]=kernel launches so far,
  * [14]=evaluations that reused a buffered list (r_buf > 0), [15] reserved. */
 mop_status mop_get_stats(mop_ctx *c, double out[16]);
 
@@ -144,7 +147,7 @@ mop_status mop_get_timing(mop_ctx *c, double out[16]);
 
 /* Copies an internal array of the last evaluation to HOST memory (synchronises).  `what`:
  *   "dims"  int[8]: nx, ny, nz (search grid), slots per bead S (padded, multiple of 32), force beads nf,
- *           cluster size 32, i-cluster size 8, 0
+ *           cluster size 8, j-clusters per warp step 4, z-bin thickness (float bits)
  *   "cell"  int[nf][Q]   cell id of every atom, cell = (cx*ny+cy)*nz+cz (reading G8)
  *   "perm"  int[nf][S]   original atom index held by each sorted slot, -1 for padding (stable sort, G13)
  *   "xq"    float[nf][S][4] wrapped coordinates + charge in sorted order
@@ -208,13 +211,21 @@ mop_status mop_add_hill(mop_ctx *c, double s_center);
  * out[4] dV/dS, out[5] number of hills; hills_host (may be NULL) receives up to cap hill centres, *n_hills their number. */
 mop_status mop_get_bias(mop_ctx *c, double out[8], double *hills_host, int cap, int *n_hills);
 
-/* Measurement aid, not part of the path: achieved FP32 rate (TFLOP/s, FMA = 2 flop) of dependent-free FMA streams
- * on all SMs of `device`, timed with CUDA events on the default stream (synchronises):
- *   out[0] scalar FFMA with a reused operand (the nominal 128 lanes/clk/SM peak of DESIGN.md section 5),
- *   out[1] scalar FFMA with three distinct register operands, out[2] packed FFMA2 (fma.rn.f32x2) with three
- *   distinct register pairs -- the operand shape of the pair kernels' FMAs; out[3] = number of SMs.
- * bench.py reports them beside the roofline.  Errors: INVALID_ARG (NULL), CUDA (no such device), OOM. */
-mop_status mop_probe_fp32(int device, double out[4]);
+/* mop_step / mop_step_langevin without the evaluation at the incoming R: the caller states that R_dev is exactly what the
+ * previous mop_step* call on this context left behind (the context still holds the gradient there), so a caller that
+ * advances a few steps per call pays n_steps evaluations per call instead of n_steps + 1.  Same results as one longer
+ * mop_step call.  Errors: INVALID_ARG when no such gradient is held (first call, or after mop_set_topology,
+ * mop_set_bias, mop_add_hill), otherwise as mop_step. */
+mop_status mop_step_continue(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps);
+mop_status mop_step_langevin_continue(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
+                                      double temperature, unsigned long long seed, unsigned long long step0);
+
+/* The production force kernel's OWN in-range decisions over the pair list of the last evaluation: its counting
+ * instance (the same code plus a population count of the per-pair results of the predicate G8 and of the exclusion
+ * masks) is run once more and the count returned in HOST *n_inrange.  which = 0: bead 1; 1: the other force beads;
+ * 2: all force beads.  This, not the scalar walker of mop_debug_pairs, is what the bit-exact neighbour-set claim of
+ * the pair kernels rests on (the tests hold it equal to the oracle's pair count).  Synchronises. */
+mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange);
 
 #ifdef __cplusplus
 }

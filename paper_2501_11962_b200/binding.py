@@ -17,7 +17,8 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
           4: "MOP_ERR_OOM", 5: "MOP_ERR_CUDA", 6: "MOP_ERR_NONFINITE"}
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
-           "mop_set_timing", "mop_get_timing", "mop_probe_fp32", "mop_eval_veff_grad_fd",
+           "mop_set_timing", "mop_get_timing", "mop_eval_veff_grad_fd", "mop_step_continue",
+           "mop_step_langevin_continue", "mop_debug_count_inrange",
            "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias"]
 
 
@@ -73,12 +74,17 @@ def load(build_if_missing=True):
     L.mop_eval_veff_grad_host.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
     L.mop_set_timing.argtypes = [C.c_void_p, C.c_int]
     L.mop_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
-    L.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    L.mop_step_continue.argtypes = L.mop_step.argtypes
+    L.mop_step_continue.restype = C.c_int
+    L.mop_debug_count_inrange.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong)]
+    L.mop_debug_count_inrange.restype = C.c_int
     L.mop_eval_veff_grad_fd.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]
     L.mop_eval_veff_grad_fd.restype = C.c_int
     L.mop_step_langevin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
                                     C.c_uint64, C.c_uint64]
     L.mop_step_langevin.restype = C.c_int
+    L.mop_step_langevin_continue.argtypes = L.mop_step_langevin.argtypes
+    L.mop_step_langevin_continue.restype = C.c_int
     L.mop_debug_noise_bits.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p]
     L.mop_debug_noise_bits.restype = C.c_int
     L.mop_set_bias.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int]
@@ -87,7 +93,6 @@ def load(build_if_missing=True):
     L.mop_add_hill.restype = C.c_int
     L.mop_get_bias.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_void_p, C.c_int, C.POINTER(C.c_int)]
     L.mop_get_bias.restype = C.c_int
-    L.mop_probe_fp32.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
         getattr(L, n).restype = C.c_int
@@ -96,10 +101,14 @@ def load(build_if_missing=True):
 
 
 def mop_probe_fp32(device=0):
-    """Achieved TFLOP/s of dependent-free FMA streams (measurement aid, include/mop.h): reused-operand FFMA,
-    three-register FFMA, three-register-pair FFMA2."""
+    """Achieved TFLOP/s of dependent-free FMA streams: reused-operand FFMA, three-register FFMA, three-register-pair
+    FFMA2.  A measurement aid for bench.py; it lives in its own small library (csrc/mop_probe.cu), not in the product."""
+    _build.build()
+    P = C.CDLL(_build.PROBE_LIB)
+    P.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
+    P.mop_probe_fp32.restype = C.c_int
     out = (C.c_double * 4)()
-    st = load().mop_probe_fp32(int(device), out)
+    st = P.mop_probe_fp32(int(device), out)
     if st != 0:
         raise MopError(st, "mop_probe_fp32 failed")
     return {"ffma_reuse_tflops": out[0], "ffma_3reg_tflops": out[1], "ffma2_3reg_tflops": out[2], "sms": int(out[3])}
@@ -230,12 +239,20 @@ class Mop:
         assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
         self._check(self.L.mop_step(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps)))
 
-    def mop_step_langevin(self, R, V, dt_pmd, n_steps, gamma, temperature, seed=0, step0=0):
-        """In-place velocity Verlet + exact OU thermostat update on torch cuda tensors R, V [N][Q][3] float32."""
+    def mop_step_continue(self, R, V, dt_pmd, n_steps):
+        """mop_step without the initial evaluation: R must be what the previous mop_step* call left behind."""
         assert R.is_cuda and V.is_cuda and R.is_contiguous() and V.is_contiguous()
         assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
-        self._check(self.L.mop_step_langevin(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps), float(gamma),
-                                             float(temperature), int(seed), int(step0)))
+        self._check(self.L.mop_step_continue(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps)))
+
+    def mop_step_langevin(self, R, V, dt_pmd, n_steps, gamma, temperature, seed=0, step0=0, cont=False):
+        """In-place velocity Verlet + exact OU thermostat update on torch cuda tensors R, V [N][Q][3] float32.
+        cont=True calls mop_step_langevin_continue (no initial evaluation)."""
+        assert R.is_cuda and V.is_cuda and R.is_contiguous() and V.is_contiguous()
+        assert tuple(R.shape) == (self.N, self.Q, 3) and tuple(V.shape) == (self.N, self.Q, 3)
+        f = self.L.mop_step_langevin_continue if cont else self.L.mop_step_langevin
+        self._check(f(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps), float(gamma), float(temperature), int(seed),
+                      int(step0)))
 
     def mop_set_bias(self, group_a, group_b, sigma, height, pace=0):
         """MoP bias on S_e2e = s(R^N) - s(R^1), s = COM distance of the two groups.  Empty groups switch it off."""
@@ -280,8 +297,8 @@ class Mop:
     def dims(self):
         d = np.zeros(8, np.int32)
         self._check(self.L.mop_debug_get(self.ctx, b"dims", d.ctypes.data_as(C.c_void_p), d.nbytes))
-        return dict(nx=int(d[0]), ny=int(d[1]), nz=int(d[2]), S=int(d[3]), nf=int(d[4]), cj=int(d[5]), ci=int(d[6]),
-                    bin_z=float(d[7:8].view(np.float32)[0]))
+        return dict(nx=int(d[0]), ny=int(d[1]), nz=int(d[2]), S=int(d[3]), nf=int(d[4]), cluster=int(d[5]),
+                    groups=int(d[6]), bin_z=float(d[7:8].view(np.float32)[0]))
 
     def mop_debug_get(self, what):
         S = self.dims()["S"]
@@ -304,6 +321,13 @@ class Mop:
         out = np.sort(out, axis=1)
         order = np.lexsort((out[:, 1], out[:, 0]))
         return out[order], int(n.value)
+
+    def mop_debug_count_inrange(self, which=2):
+        """In-range, non-excluded pair decisions of the PRODUCTION force kernel (counting instance) over the list of
+        the last evaluation.  which: 0 bead 1, 1 the other force beads, 2 all force beads."""
+        n = C.c_longlong(0)
+        self._check(self.L.mop_debug_count_inrange(self.ctx, int(which), C.byref(n)))
+        return int(n.value)
 
     def mop_destroy(self):
         if getattr(self, "ctx", None) is not None and self.ctx.value:

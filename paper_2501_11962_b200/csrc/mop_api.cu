@@ -17,7 +17,6 @@
 #include "mop_nonbonded_packed.cuh"
 #include "mop_pairlist.cuh"
 #include "mop_path.cuh"
-#include "mop_probe.cuh"
 
 static thread_local char g_create_error[256] = "";
 
@@ -45,11 +44,11 @@ struct mop_ctx {
     // per-bead sorted state
     int *d_cell = 0, *d_cell_count = 0, *d_cell_rel = 0, *d_cell_fill = 0, *d_col_count = 0, *d_col_start = 0;
     int *d_tmp = 0, *d_perm = 0, *d_slot_of = 0, *d_typ = 0;
-    float4 *d_xq = 0, *d_et = 0, *d_F4 = 0, *d_H4 = 0, *d_jlo = 0, *d_jhi = 0, *d_ilo = 0, *d_ihi = 0;
+    float4 *d_xq = 0, *d_et = 0, *d_F4 = 0, *d_H4 = 0, *d_blo = 0, *d_bhi = 0;
     // pair list
     MopUnit *d_units = 0;
     MopEntry *d_entries = 0;
-    unsigned *d_masks = 0;
+    unsigned long long *d_masks = 0;
     unsigned cap_units = 0, cap_entries = 0, cap_masks = 0;
     MopCounters *d_ctr = 0;
     unsigned long long *d_slots = 0;
@@ -62,8 +61,9 @@ struct mop_ctx {
     // scratch
     float *d_G = 0;     // [N][Q][3] gradient for mop_step
     float *d_dbg = 0;   // [nf][Q][3]
-    int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0;
-    int var_f = 2, var_h = 2;   // tuning variants of the pair kernels (NBP_* flags; 2 = five CTAs per SM)
+    int nb_blocks_f = 0, nb_blocks_fe = 0, nb_blocks_h = 0, nb_blocks_c = 0;
+    bool caps_checked = false;  // the list capacities have been checked against one real build (first evaluation)
+    bool g_current = false;     // d_G holds the gradient at the R the last mop_step* call returned (mop_step_continue)
     double last_veff = 0, last_ekin = 0;
     // e2e staging (mop_eval_veff_grad_host)
     float *d_Rh = 0, *d_Gh = 0;
@@ -128,17 +128,14 @@ static cudaError_t dalloc(T **p, size_t n) {
 static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 typedef void (*nb_kernel_t)(const NbArgs);
-// tuning variants of the pair kernels: NBP_* flags (mop_nonbonded_packed.cuh); MOP_NB_VAR / MOP_NB_VAR_H override
-#define NBP_VARIANTS(MODE)                                                                                    \
-    {k_nonbonded_p<MODE, 0>, k_nonbonded_p<MODE, 1>, k_nonbonded_p<MODE, 2>, k_nonbonded_p<MODE, 3>,          \
-     k_nonbonded_p<MODE, 4>, k_nonbonded_p<MODE, 5>, k_nonbonded_p<MODE, 6>, k_nonbonded_p<MODE, 7>}
-static const nb_kernel_t k_force_p[8] = NBP_VARIANTS(NB_FORCE);
-static const nb_kernel_t k_energy_p[8] = NBP_VARIANTS(NB_ENERGY);
-static const nb_kernel_t k_hvp_p[8] = NBP_VARIANTS(NB_HVP);
-static size_t nb_smem(const mop_ctx *c, int) { return nbp_smem_bytes(c->nt); }
-static nb_kernel_t nb_pick(int mode, int var) {
-    return (mode == NB_FORCE ? k_force_p : mode == NB_ENERGY ? k_energy_p : k_hvp_p)[var & 7];
+// the launched instances of the pair kernel (five resident CTAs per SM: 96 registers)
+#define NBP_CTAS 5
+static nb_kernel_t nb_pick(int mode, bool count = false) {
+    if (count) return k_nonbonded_p<NB_FORCE, true, NBP_CTAS>;
+    return mode == NB_FORCE ? k_nonbonded_p<NB_FORCE, false, NBP_CTAS>
+         : mode == NB_ENERGY ? k_nonbonded_p<NB_ENERGY, false, NBP_CTAS> : k_nonbonded_p<NB_HVP, false, NBP_CTAS>;
 }
+static size_t nb_smem(const mop_ctx *c) { return nbp_smem_bytes(c->nt); }
 
 extern "C" const char *mop_last_error(const mop_ctx *c) { return c ? c->err.c_str() : g_create_error; }
 
@@ -147,8 +144,8 @@ static void free_all(mop_ctx *c) {
                     c->d_tab,     c->d_bond_par, c->d_angle_par, c->d_type_row,  c->d_bond_ij,  c->d_angle_ijk,
                     c->d_excl_start, c->d_excl_list, c->d_cell,  c->d_cell_count, c->d_cell_rel, c->d_cell_fill,
                     c->d_col_count, c->d_col_start, c->d_tmp,    c->d_perm,      c->d_slot_of,  c->d_typ,
-                    c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_jlo,      c->d_jhi,
-                    c->d_ilo,     c->d_ihi,      c->d_units,     c->d_entries,   c->d_masks,    c->d_ctr,
+                    c->d_xq,      c->d_et,       c->d_F4,        c->d_H4,        c->d_blo,      c->d_bhi,
+                    c->d_units,   c->d_entries,  c->d_masks,     c->d_ctr,
                     c->d_slots,   c->d_work,     c->d_energy,    c->d_G,         c->d_dbg,       c->d_Rh,
                     c->d_Gh,      c->d_fdR,      c->d_fdEta,     c->d_fdF,       c->d_fdFp,     c->d_fdFm,
                     c->d_Rref,    c->d_moved,
@@ -215,16 +212,16 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
         c->krf = (float)krf;
         c->crf = (float)(1.0 / rc + krf * rc * rc);
     }
-    // search grid (S0): columns of side ~ (32/rho)^(1/3) in x,y; thin bins of side/12 along z
+    // search grid (S0): columns of side ~ (8/rho)^(1/3) in x,y; thin bins of side/8 along z
     MopGrid &g = c->g;
     {
         double vol = (double)p->box[0] * (double)p->box[1] * (double)p->box[2];
-        double side = cbrt((double)MOP_CJ * vol / (double)c->Q);
+        double side = cbrt((double)MOP_CL * vol / (double)c->Q);
         for (int d = 0; d < 2; d++) {
             int n = (int)floor((double)p->box[d] / side);
             g.dims[d] = n < 1 ? 1 : (n > 1024 ? 1024 : n);
         }
-        c->bin_z = (float)(side / 12.0);
+        c->bin_z = (float)(side / 8.0);
         int nz = (int)floor((double)p->box[2] / (double)c->bin_z);
         g.dims[2] = nz < 1 ? 1 : (nz > 4096 ? 4096 : nz);
         for (int d = 0; d < 3; d++) {
@@ -238,7 +235,7 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
         g.colw[1] = p->box[1] / (float)g.dims[1];
         g.Q = c->Q;
         g.nf = c->nf;
-        size_t S = (size_t)c->Q + 31u * (size_t)g.ncol;
+        size_t S = (size_t)c->Q + (size_t)(MOP_CL - 1) * (size_t)g.ncol;
         g.S = (int)((S + 31) / 32 * 32);
     }
     const size_t nf = c->nf, Q = c->Q, S = g.S;
@@ -260,10 +257,8 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     A(dalloc(&c->d_et, nf * S));
     A(dalloc(&c->d_F4, nf * S));
     A(dalloc(&c->d_H4, nf * S));
-    A(dalloc(&c->d_jlo, nf * S / MOP_CJ));
-    A(dalloc(&c->d_jhi, nf * S / MOP_CJ));
-    A(dalloc(&c->d_ilo, nf * S / MOP_CI));
-    A(dalloc(&c->d_ihi, nf * S / MOP_CI));
+    A(dalloc(&c->d_blo, nf * S / MOP_CL));
+    A(dalloc(&c->d_bhi, nf * S / MOP_CL));
     A(dalloc(&c->d_ctr, 1));
     A(dalloc(&c->d_slots, 1));
     A(dalloc(&c->d_work, 8));
@@ -286,6 +281,17 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     memset(c->h_ctr, 0, sizeof(MopCounters));
     *c->h_slots = 0;
     *out = c;
+    return MOP_OK;
+}
+
+// (re)allocates the pair-list buffers for at least the given numbers of units, entries and exclusion-mask rows
+static mop_status alloc_lists(mop_ctx *c, double units, double entries, double masks) {
+    auto cap = [](double v) { return (unsigned)std::min(std::max(v, 64.0), 3.5e9); };
+    c->cap_units = cap(units), c->cap_entries = cap(entries), c->cap_masks = cap(masks);
+    CK(c, dalloc(&c->d_units, (size_t)c->cap_units));
+    CK(c, dalloc(&c->d_entries, (size_t)c->cap_entries));
+    CK(c, dalloc(&c->d_masks, (size_t)c->cap_masks));
+    c->list_valid = false;
     return MOP_OK;
 }
 
@@ -394,41 +400,29 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
         if (c->d_excl_start) cudaFree(c->d_excl_start), c->d_excl_start = nullptr;
         if (c->d_excl_list) cudaFree(c->d_excl_list), c->d_excl_list = nullptr;
     }
-    // pair-list capacities (S1): volume bound on cluster pairs per i-cluster, with head room
+    // pair-list capacities (S1): one unit per i-octet (exact bound); entries from the volume of the
+    // half shell of octets within reach, masks from the exclusion count, both with head room.  The first evaluation
+    // checks them against a real build and regrows them if the estimate was short (inhomogeneous systems).
     {
         const MopGrid &g = c->g;
+        const double kPi = 3.14159265358979;
         double vol = (double)g.box[0] * g.box[1] * g.box[2];
-        double side = cbrt((double)MOP_CJ * vol / (double)Q);
-        double reach = 2.0 * c->rl + 2.0 * side;
-        double per_ci = 0.5 * ((double)Q / MOP_CJ / vol) * reach * reach * reach * 1.3;
-        if (per_ci < 64.0) per_ci = 64.0;
-        double nci = (double)c->nf * g.S / MOP_CI;
-        double ce = nci * per_ci;
-        if (ce > 3.5e9) ce = 3.5e9;
-        c->cap_entries = (unsigned)ce;
-        bool tiny = false;
-        for (int d = 0; d < 3; d++)
-            if (g.box[d] < 4.0f * c->rl) tiny = true;
-        double cu = nci * (tiny ? 27.0 : 4.0);
-        if (cu > 3.5e9) cu = 3.5e9;
-        c->cap_units = (unsigned)cu;
-        int rows = 1 + (max_excl > 0 ? std::min(12, 2 * max_excl + 2) : 0);
-        double cm = nci * rows;
-        if (cm > 3.5e9) cm = 3.5e9;
-        c->cap_masks = (unsigned)cm;
-        CK(c, dalloc(&c->d_units, (size_t)c->cap_units));
-        CK(c, dalloc(&c->d_entries, (size_t)c->cap_entries));
-        CK(c, dalloc(&c->d_masks, (size_t)c->cap_masks * MOP_CI));
+        double side = cbrt((double)MOP_CL * vol / (double)Q);
+        double reach = c->rl + 1.2 * side;
+        double per_ci = 0.5 * ((double)Q / MOP_CL / vol) * (4.0 / 3.0) * kPi * reach * reach * reach * 1.25 + 16.0;
+        double nci = (double)c->nf * g.S / MOP_CL;
+        int rows = 1 + (max_excl > 0 ? std::min(MOP_EXROWS - 1, 2 * max_excl + 2) : 0);
+        mop_status st = alloc_lists(c, nci, nci * per_ci, nci * rows);
+        if (st) return st;
+        c->caps_checked = false;
     }
     // launch geometry of the persistent pair kernels
     {
-        if (const char *ev = getenv("MOP_NB_VAR")) c->var_f = c->var_h = atoi(ev) & 7;
-        if (const char *ev = getenv("MOP_NB_VAR_H")) c->var_h = atoi(ev) & 7;
-        const void *fns[3] = {(const void *)nb_pick(NB_FORCE, c->var_f), (const void *)nb_pick(NB_ENERGY, c->var_f),
-                              (const void *)nb_pick(NB_HVP, c->var_h)};
-        int *nbs[3] = {&c->nb_blocks_f, &c->nb_blocks_fe, &c->nb_blocks_h};
-        for (int k = 0; k < 3; k++) {
-            const size_t smem = nb_smem(c, k == 2 ? c->var_h : c->var_f);
+        const void *fns[4] = {(const void *)nb_pick(NB_FORCE), (const void *)nb_pick(NB_ENERGY), (const void *)nb_pick(NB_HVP),
+                              (const void *)nb_pick(NB_FORCE, true)};
+        int *nbs[4] = {&c->nb_blocks_f, &c->nb_blocks_fe, &c->nb_blocks_h, &c->nb_blocks_c};
+        for (int k = 0; k < 4; k++) {
+            const size_t smem = nb_smem(c);
             CK(c, cudaFuncSetAttribute(fns[k], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             int b = 0;
             CK(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, fns[k], 128, smem));
@@ -438,6 +432,7 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     CK(c, cudaStreamSynchronize(c->st));
     c->has_topology = true;
     c->list_valid = false;
+    c->g_current = false;
     return MOP_OK;
 }
 
@@ -465,39 +460,44 @@ static void t_mark(mop_ctx *c, int k) {
 }
 
 // ---- S0 + S1 for the first nb beads of R ----
-static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = false) {
+// per-build counters start from zero; the overflow and non-finite words are sticky (only a regrow clears overflow)
+__global__ void k_ctr_reset(MopCounters *ctr, unsigned long long *slots) {
+    ctr->n_units = ctr->n_entries = ctr->n_masks = ctr->n_units_bead0 = 0u;
+    *slots = 0ull;
+}
+__global__ void k_ctr_clear_overflow(MopCounters *ctr) { ctr->overflow = 0u; }
+
+static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed) {
     const MopGrid &g = c->g;
     const size_t Q = c->Q;
     CK(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
     CK(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
-    CK(c, cudaMemsetAsync(c->d_ctr, 0, sizeof(MopCounters), c->st));
-    CK(c, cudaMemsetAsync(c->d_slots, 0, sizeof(unsigned long long), c->st));
+    LAUNCH(c, k_ctr_reset, 1, 1, 0, c->d_ctr, c->d_slots);
     dim3 ga(cdiv(Q, 256), nb), gs(cdiv(g.S, 256), nb);
-    LAUNCH(c, k_bin, ga, 256, 0, R, g, c->d_cell, c->d_cell_count);
+    LAUNCH(c, k_bin, ga, 256, 0, R, g, c->d_cell, c->d_cell_count, &c->d_ctr->nonfinite);
     LAUNCH(c, k_colscan, dim3(cdiv(g.ncol, 4), nb), 128, 0, g, c->d_cell_count, c->d_cell_rel, c->d_col_count);
     LAUNCH(c, k_colstart, nb, 1024, 0, g, c->d_col_count, c->d_col_start);
     LAUNCH(c, k_fill_pad, gs, 256, 0, g, c->d_perm, c->d_xq, c->d_typ);
     LAUNCH(c, k_place, ga, 256, 0, g, c->d_cell, c->d_cell_rel, c->d_col_start, c->d_cell_fill, c->d_tmp);
     LAUNCH(c, k_rank, ga, 256, 0, R, g, c->d_cell, c->d_cell_rel, c->d_col_start, c->d_cell_count, c->d_tmp,
            c->d_charge, c->d_type_row, c->d_perm, c->d_slot_of, c->d_xq, c->d_typ);
-    LAUNCH(c, k_bbox, dim3(cdiv(g.S / MOP_CJ, 4), nb), 128, 0, g, c->d_perm, c->d_xq, c->d_jlo, c->d_jhi, c->d_ilo,
-           c->d_ihi);
+    LAUNCH(c, k_bbox, dim3(cdiv(g.S, 128), nb), 128, 0, g, c->d_perm, c->d_xq, c->d_blo, c->d_bhi);
     if (timed) t_mark(c, 1);
     PlArgs a;
     a.g = g;
     a.rl = c->rl;
     a.rl2 = c->rl2;
     a.perm = c->d_perm, a.slot_of = c->d_slot_of, a.xq = c->d_xq;
-    a.jlo = c->d_jlo, a.jhi = c->d_jhi, a.ilo = c->d_ilo, a.ihi = c->d_ihi;
+    a.blo = c->d_blo, a.bhi = c->d_bhi;
     a.col_start = c->d_col_start, a.cell_rel = c->d_cell_rel, a.col_count = c->d_col_count;
     a.excl_start = c->d_excl_start, a.excl_list = c->d_excl_list;
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.slots_active = c->d_slots;
     a.cap_units = c->cap_units, a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks;
-    const unsigned nci_blocks = cdiv(g.S / MOP_CI, 4);
+    const unsigned nci_blocks = cdiv(g.S / MOP_CL, 4);
     a.bead0 = 0;
     LAUNCH(c, k_pairlist, dim3(nci_blocks, 1), 128, 0, a); // bead 1 first: its units come first (energy variant)
-    LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr);
+    LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr, c->cap_units);
     if (nb > 1) {
         a.bead0 = 1;
         LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 128, 0, a);
@@ -508,6 +508,33 @@ static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = fa
     return MOP_OK;
 }
 
+// the builder keeps counting past the capacities, so an overflowed build tells what a sufficient allocation is
+static mop_status regrow_lists(mop_ctx *c) {
+    const MopCounters &h = *c->h_ctr;
+    const double nu = std::max((double)c->cap_units, 1.05 * h.n_units), ne = std::max((double)c->cap_entries, 1.3 * h.n_entries),
+                 nm = std::max((double)c->cap_masks, 1.3 * h.n_masks);
+    if (h.overflow & 24u) FAIL(c, MOP_ERR_OOM, "pair-list builder: per-octet staging (8) or exclusion rows (16) exhausted, flags 0x%x", h.overflow);
+    CK(c, cudaStreamSynchronize(c->st));
+    mop_status s = alloc_lists(c, nu, ne, nm);
+    if (s) return s;
+    LAUNCH(c, k_ctr_clear_overflow, 1, 1, 0, c->d_ctr);
+    return MOP_OK;
+}
+
+static mop_status build_list(mop_ctx *c, const float *R, int nb, bool timed = false) {
+    mop_status s = build_list_once(c, R, nb, timed);
+    if (s || c->caps_checked) return s;
+    // first build with these capacities: check them on the host (one synchronisation per topology), regrow and rebuild
+    for (int attempt = 0; attempt < 3; attempt++) {
+        CK(c, cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st));
+        CK(c, cudaStreamSynchronize(c->st));
+        if (!c->h_ctr->overflow) break;
+        if ((s = regrow_lists(c))) return s;
+        if ((s = build_list_once(c, R, nb, false))) return s;
+    }
+    c->caps_checked = true;
+    return MOP_OK;
+}
 
 static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     NbArgs a;
@@ -516,6 +543,8 @@ static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     a.k2rf = 2.0f * c->krf, a.krf = c->krf, a.crf = c->crf;
     a.xq = c->d_xq, a.typ = c->d_typ, a.et = c->d_et, a.out = out;
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
+    a.cap_units = c->cap_units;
+    a.n_inrange = &c->d_ctr->n_inrange;
     a.work = c->d_work + work_slot;
     a.range = range;
     a.tab = c->d_tab, a.tabs = c->d_tabs;
@@ -537,13 +566,13 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
 // pass 1 on the first nb beads: nonbonded (energy variant on bead 1) + bonded.  with_energy = false (displaced
 // configurations of the finite-difference mode): plain force kernel on every bead, energy sums go to scratch
 static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false, bool with_energy = true) {
-    const size_t smem = nb_smem(c, c->var_f);
+    const size_t smem = nb_smem(c);
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
     if (with_energy) {
-        LAUNCH(c, nb_pick(NB_ENERGY, c->var_f), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
-        if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
+        LAUNCH(c, nb_pick(NB_ENERGY), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
+        if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
     } else {
-        LAUNCH(c, nb_pick(NB_FORCE, c->var_f), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 0, 2));
+        LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 0, 2));
     }
     if (timed) t_mark(c, 3);
     const int nterm = c->n_bonds + c->n_angles;
@@ -558,9 +587,9 @@ static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = fa
 
 // pass 2 on the first nb beads: nonbonded + bonded Hessian-vector product with the direction held in et
 static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = false) {
-    const size_t smem = nb_smem(c, c->var_h);
+    const size_t smem = nb_smem(c);
     CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
-    LAUNCH(c, nb_pick(NB_HVP, c->var_h), c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
+    LAUNCH(c, nb_pick(NB_HVP), c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
     if (timed) t_mark(c, 6);
     const int nterm = c->n_bonds + c->n_angles;
     if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));
@@ -574,10 +603,20 @@ static mop_status read_back(mop_ctx *c) {
     CK(c, cudaMemcpyAsync(c->h_slots, c->d_slots, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaStreamSynchronize(c->st));
     CK(c, cudaGetLastError());
+    if (c->h_ctr->nonfinite) {
+        c->sticky = MOP_ERR_NONFINITE;
+        FAIL(c, MOP_ERR_NONFINITE, "a coordinate is NaN/Inf or farther than ~1e6 box lengths from the box");
+    }
     if (c->h_ctr->overflow) {
-        c->sticky = MOP_ERR_OOM;
-        FAIL(c, MOP_ERR_OOM, "pair-list buffer overflow (flags 0x%x: 1 entries, 2 units, 4 masks, 8 staging, 16 excl rows)",
-             c->h_ctr->overflow);
+        // some build since the last check dropped pairs: the results of this call are invalid.  The buffers are
+        // regrown from the builder's own counts, so the caller can simply repeat the evaluation.
+        const unsigned fl = c->h_ctr->overflow;
+        mop_status s = regrow_lists(c);
+        if (s) {
+            c->sticky = s;
+            return s;
+        }
+        FAIL(c, MOP_ERR_OOM, "pair-list buffer overflow (flags 0x%x: 1 entries, 2 units, 4 masks); buffers regrown, repeat the call", fl);
     }
     const double *E = c->h_energy;
     c->last_veff = E[0] + E[1] + E[2] + E[3] + E[4];
@@ -765,44 +804,21 @@ extern "C" mop_status mop_get_timing(mop_ctx *c, double out[16]) {
     return MOP_OK;
 }
 
-extern "C" mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps) {
-    PRECHECK(c);
+// velocity Verlet on eq. (4) (+ the exact OU velocity update when ou); cont: d_G already holds the gradient at R_dev
+static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, bool cont, bool ou, double cc,
+                            float amp, unsigned long long seed, unsigned long long step0) {
     if (!R_dev || !V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or V_dev is NULL");
     if (n_steps < 0 || !(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
     const size_t total = (size_t)c->N * c->Q * 3;
     if (!c->d_G) CK(c, dalloc(&c->d_G, total));
-    mop_status s = eval_async(c, R_dev, c->d_G);
-    if (s) return s;
-    const unsigned nblk = cdiv(total, 256);
-    for (int it = 0; it < n_steps; it++) {
-        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
-               (double *)nullptr);
-        c->bias_steps += 1;
-        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0))) return s;
-        const bool last = it == n_steps - 1;
-        if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
-        LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
-               last ? c->d_energy + 5 : (double *)nullptr);
+    mop_status s;
+    if (cont) {
+        if (!c->g_current) FAIL(c, MOP_ERR_INVALID_ARG, "mop_step*_continue: no gradient from a previous mop_step* call is held");
+    } else if ((s = eval_async(c, R_dev, c->d_G))) {
+        return s;
     }
-    CK(c, cudaGetLastError());
-    return MOP_OK;
-}
-
-// path MD with the Langevin thermostat of the paper's NVT runs: velocity Verlet, then the exact OU velocity update
-extern "C" mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
-                                        double temperature, unsigned long long seed, unsigned long long step0) {
-    PRECHECK(c);
-    if (!R_dev || !V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or V_dev is NULL");
-    if (n_steps < 0 || !(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
-    if (!(gamma >= 0.0) || !(temperature >= 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need gamma >= 0 and temperature >= 0");
-    const size_t total = (size_t)c->N * c->Q * 3;
-    if (!c->d_G) CK(c, dalloc(&c->d_G, total));
-    mop_status s = eval_async(c, R_dev, c->d_G);
-    if (s) return s;
+    c->g_current = false;
     const unsigned nblk = cdiv(total, 256);
-    const double cc = exp(-gamma * dt_pmd);
-    const float amp = (float)sqrt((1.0 - cc * cc) * 0.0083144626 * temperature);   // k_B in kJ mol^-1 K^-1
-    const bool ou = gamma > 0.0;
     for (int it = 0; it < n_steps; it++) {
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (double *)nullptr);
@@ -817,7 +833,41 @@ extern "C" mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, 
                    c->d_mass, V_dev, last ? c->d_energy + 5 : (double *)nullptr);
     }
     CK(c, cudaGetLastError());
+    c->g_current = true;   // d_G is the gradient at the R_dev this call leaves behind
     return MOP_OK;
+}
+
+extern "C" mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps) {
+    PRECHECK(c);
+    return step_impl(c, R_dev, V_dev, dt_pmd, n_steps, false, false, 1.0, 0.f, 0ull, 0ull);
+}
+
+extern "C" mop_status mop_step_continue(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps) {
+    PRECHECK(c);
+    return step_impl(c, R_dev, V_dev, dt_pmd, n_steps, true, false, 1.0, 0.f, 0ull, 0ull);
+}
+
+// path MD with the Langevin thermostat of the paper's NVT runs: velocity Verlet, then the exact OU velocity update
+static mop_status langevin_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
+                                double temperature, unsigned long long seed, unsigned long long step0, bool cont) {
+    if (!(gamma >= 0.0) || !(temperature >= 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need gamma >= 0 and temperature >= 0");
+    if (!(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
+    const double cc = exp(-gamma * dt_pmd);
+    const float amp = (float)sqrt((1.0 - cc * cc) * 0.0083144626 * temperature);   // k_B in kJ mol^-1 K^-1
+    return step_impl(c, R_dev, V_dev, dt_pmd, n_steps, cont, gamma > 0.0, cc, amp, seed, step0);
+}
+
+extern "C" mop_status mop_step_langevin(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, double gamma,
+                                        double temperature, unsigned long long seed, unsigned long long step0) {
+    PRECHECK(c);
+    return langevin_impl(c, R_dev, V_dev, dt_pmd, n_steps, gamma, temperature, seed, step0, false);
+}
+
+extern "C" mop_status mop_step_langevin_continue(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps,
+                                                 double gamma, double temperature, unsigned long long seed,
+                                                 unsigned long long step0) {
+    PRECHECK(c);
+    return langevin_impl(c, R_dev, V_dev, dt_pmd, n_steps, gamma, temperature, seed, step0, true);
 }
 
 // debug: raw bits of the thermostat's counter-based generator for idx = 0..n-1 (HOST output)
@@ -843,6 +893,7 @@ extern "C" mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, cons
     CK(c, cudaStreamSynchronize(c->st));
     c->bias_on = false;
     c->bias_steps = 0;
+    c->g_current = false;
     if (n_a == 0 && n_b == 0) return MOP_OK;   // bias switched off
     if (n_a < 1 || n_b < 1 || !group_a || !group_b) FAIL(c, MOP_ERR_INVALID_ARG, "mop_set_bias: both groups need atoms");
     if (!(sigma > 0.0) || !std::isfinite(height) || pace < 0) FAIL(c, MOP_ERR_INVALID_ARG, "need sigma > 0, finite height, pace >= 0");
@@ -872,6 +923,7 @@ extern "C" mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, cons
 extern "C" mop_status mop_add_hill(mop_ctx *c, double s_center) {
     PRECHECK(c);
     if (!c->bias_on) FAIL(c, MOP_ERR_INVALID_ARG, "mop_add_hill: no bias set");
+    c->g_current = false;
     int nh = 0;
     CK(c, cudaMemcpyAsync(&nh, c->d_bias_nh, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaStreamSynchronize(c->st));
@@ -919,7 +971,7 @@ extern "C" mop_status mop_get_stats(mop_ctx *c, double out[16]) {
     out[9] = (double)c->h_ctr->n_entries;
     out[10] = (double)c->h_ctr->n_units;
     out[11] = (double)c->h_ctr->n_masks;
-    out[12] = (double)(*c->h_slots) * 32.0;
+    out[12] = (double)(*c->h_slots);
     out[13] = c->n_launches;
     out[14] = c->n_reuses;
     out[15] = 0.0;
@@ -939,7 +991,7 @@ extern "C" mop_status mop_debug_get(mop_ctx *c, const char *what, void *host_buf
         return MOP_OK;
     };
     if (w == "dims") {
-        int d[8] = {g.dims[0], g.dims[1], g.dims[2], g.S, c->nf, MOP_CJ, MOP_CI, 0};
+        int d[8] = {g.dims[0], g.dims[1], g.dims[2], g.S, c->nf, MOP_CL, MOP_NG, 0};
         memcpy(&d[7], &c->bin_z, 4);
         if (bytes != sizeof d) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_get(dims): expected %zu bytes", sizeof d);
         memcpy(host_buf, d, sizeof d);
@@ -967,7 +1019,7 @@ extern "C" mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long lon
     PairDbgArgs a;
     a.S = c->g.S, a.bead = bead, a.rc2 = c->rc2;
     a.xq = c->d_xq, a.perm = c->d_perm, a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks;
-    a.ctr = c->d_ctr, a.pairs = d_pairs, a.cap = cap;
+    a.ctr = c->d_ctr, a.cap_units = c->cap_units, a.pairs = d_pairs, a.cap = cap;
     for (int d = 0; d < 3; d++) a.box[d] = c->g.box[d];
     cudaMemsetAsync(&c->d_ctr->n_pairs, 0, sizeof(unsigned long long), c->st);
     LAUNCH(c, k_debug_pairs, c->sm_count * 8, 128, 0, a);
@@ -980,6 +1032,23 @@ extern "C" mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long lon
     }
     cudaFree(d_pairs);
     CK(c, e);
+    return MOP_OK;
+}
+
+// The production force kernel's own in-range decisions (its counting instance: same code, plus a population count
+// of the per-pair predicate results) over the list of the last evaluation.  which = 0: bead 1; 1: the other force
+// beads; 2: all force beads.  The forces it computes go to the H.eta scratch array.  Synchronises.
+extern "C" mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange) {
+    PRECHECK(c);
+    if (which < 0 || which > 2 || !n_inrange) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_count_inrange: bad argument");
+    if (c->n_rebuilds == 0) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_count_inrange: no evaluation yet");
+    CK(c, cudaMemsetAsync(&c->d_ctr->n_inrange, 0, sizeof(unsigned long long), c->st));
+    CK(c, cudaMemsetAsync(c->d_work + 3, 0, sizeof(unsigned), c->st));
+    LAUNCH(c, nb_pick(NB_FORCE, true), c->nb_blocks_c, 128, nb_smem(c), nb_args(c, c->d_H4, 3, which));
+    CK(c, cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaStreamSynchronize(c->st));
+    CK(c, cudaGetLastError());
+    *n_inrange = (long long)c->h_ctr->n_inrange;
     return MOP_OK;
 }
 
@@ -1004,38 +1073,3 @@ extern "C" mop_status mop_force_hvp(mop_ctx *c, const float *R_dev, const float 
     return MOP_OK;
 }
 
-// FP32-pipe probe (measurement aid): TFLOP/s of dependent-free FMA streams, FMA = 2 flop
-extern "C" mop_status mop_probe_fp32(int device, double out[4]) {
-    if (!out) return MOP_ERR_INVALID_ARG;
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev || cudaSetDevice(device) != cudaSuccess) {
-        cudaGetLastError();
-        return MOP_ERR_CUDA;
-    }
-    int sms = 0;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
-    const int grid = sms * 4, block = 256;
-    float *buf = nullptr;
-    if (cudaMalloc((void **)&buf, (size_t)grid * block * sizeof(float)) != cudaSuccess) return MOP_ERR_OOM;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0), cudaEventCreate(&e1);
-    void (*ks[3])(float *, float) = {k_probe_fp32<0>, k_probe_fp32<1>, k_probe_fp32<2>};
-    const double fma_per_thread[3] = {8.0 * MOP_PROBE_ITER, 8.0 * MOP_PROBE_ITER, 16.0 * MOP_PROBE_ITER};
-    for (int m = 0; m < 3; m++) {
-        float best = 1e30f;
-        for (int rep = 0; rep < 4; rep++) {
-            cudaEventRecord(e0);
-            ks[m]<<<grid, block>>>(buf, 1.0001f);
-            cudaEventRecord(e1);
-            cudaEventSynchronize(e1);
-            float ms = 0.f;
-            cudaEventElapsedTime(&ms, e0, e1);
-            if (rep > 0 && ms < best) best = ms;
-        }
-        out[m] = 2.0 * fma_per_thread[m] * (double)grid * block / (best * 1e-3) / 1e12;
-    }
-    out[3] = (double)sms;
-    cudaEventDestroy(e0), cudaEventDestroy(e1);
-    cudaFree(buf);
-    return cudaGetLastError() == cudaSuccess ? MOP_OK : MOP_ERR_CUDA;
-}

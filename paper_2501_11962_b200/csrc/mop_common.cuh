@@ -1,23 +1,25 @@
 // mop_common.cuh -- shared declarations of the CUDA hot path (sm_100a).
 //
 // Data layout in HBM (per force bead n < nf, nf = max(N-1,1); S = padded slots per bead):
-//   xq   [nf][S] float4  wrapped coordinates + charge, sorted by (column, z-bin), columns padded to 32
+//   xq   [nf][S] float4  wrapped coordinates + charge, sorted by (column, z-bin), columns padded to 8
 //   typ  [nf][S] int     type * n_types (row offset into the LJ table), sorted order
 //   et   [nf][S] float4  eta^n (xyz) + type row offset (w, int bits), sorted order, pass-2 input
 //   F4   [nf][S] float4  physical force F^n, sorted order (w unused)
 //   H4   [nf][S] float4  H^n eta^n, sorted order (w unused)
 //   perm [nf][S] int     sorted slot -> original atom (-1: padding);  slot_of [nf][Q] the inverse
-// j-cluster = 32 consecutive slots (one warp lane each); i-cluster = 8 consecutive slots.
+// A cluster ("octet") = 8 consecutive slots: a compact group of ~8 atoms (thin x,y columns of side ~ (8/rho)^(1/3),
+// sorted along z).  The same octets serve as i-clusters (one work unit each) and as j-clusters (four per warp step).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define MOP_CJ 32          // atoms per j-cluster (= warp lanes)
-#define MOP_CI 8           // atoms per i-cluster (processed sequentially by one warp)
+#define MOP_CL 8           // atoms per cluster (octet)
+#define MOP_NG 4           // j-octets per warp step (lane = (j atom 0..7, group 0..3))
 #define MOP_KE 138.935458f // Coulomb constant, kJ mol^-1 nm e^-2
 #define MOP_MAX_TYPES 64
-#define MOP_EXROWS 32      // max distinct j-clusters holding exclusion partners of one i-cluster
-#define MOP_LBUF 448       // per-warp staging capacity (cluster-pair entries) in the list builder
+#define MOP_EXROWS 48      // max distinct j-octets holding exclusion partners of one i-octet (row 0: the octet itself)
+#define MOP_LBUF 512       // per-warp staging capacity (candidate j-octets) in the list builder
+#define MOP_NOSHIFT 13     // shift id (kx+1) + 3 (ky+1) + 9 (kz+1) of the zero shift
 
 struct MopGrid {
     float box[3], inv_box[3]; // inv_box = 1.0f / box (FP32)
@@ -29,23 +31,25 @@ struct MopGrid {
     float colw[2];            // column widths box/dims
 };
 
-struct MopUnit {            // one work unit of the pair kernels: (bead, i-cluster, periodic shift)
+struct MopUnit {            // one work unit of the pair kernels: (bead, i-octet)
     int bead;
-    int ci;                 // i-cluster index within the bead (slot = ci*8 + k)
-    int shift;              // (kx+1) + 3*(ky+1) + 9*(kz+1); 13 = no shift
-    unsigned start, count;  // range in the entry array
-    unsigned excl_base;     // first exclusion-mask row of this i-cluster
-    unsigned pad0, pad1;
+    int ci;                 // i-octet index within the bead (slot = ci*8 + k)
+    unsigned start, count;  // range in the entry array; count is a multiple of MOP_NG (padded with pattern-0 entries)
+    unsigned excl_base;     // first exclusion-mask row of this i-octet
+    unsigned pad0, pad1, pad2;
 };
 
-// entry: x = j-cluster index within the bead; y = imask (bits 0-7: which i atoms can be in range)
-//        | (exclusion row + 1) << 8 (0: no exclusions in this cluster pair)
+// entry: x = j-octet index within the bead | shift id << 24  ((kx+1) + 3 (ky+1) + 9 (kz+1), MOP_NOSHIFT = none)
+//        y = pattern (bits 0-3: row pair p = i atoms (2p, 2p+1) has a pair within r_list of this octet; 0: padding)
+//            | (exclusion row + 1) << 8 (0: no exclusions in this octet pair)
+// The entries of a unit are ordered by pattern, so that the four octets of a warp step mostly share theirs.
 typedef uint2 MopEntry;
 
 struct MopCounters {
     unsigned n_units, n_entries, n_masks, overflow; // overflow: bit0 entries, bit1 units, bit2 masks, bit3 staging, bit4 excl rows
-    unsigned n_units_bead0, work0, work1, pad;
-    unsigned long long n_pairs; // debug pair walker
+    unsigned n_units_bead0, nonfinite, work1, pad;  // nonfinite: an input coordinate was NaN/Inf or beyond 1e6 box lengths
+    unsigned long long n_pairs;   // debug pair walker
+    unsigned long long n_inrange; // in-range decisions counted by the production force kernel (counting variant)
 };
 
 // ---- G8: the FP32 expressions shared by every kernel that classifies (fixed order, never contracted) ----
@@ -59,15 +63,21 @@ __device__ __forceinline__ float mop_wrap1(float x, float L, float invL) {
     return xw;
 }
 
+// clamped on both sides: a coordinate the wrap could not bring into [0, L) (|x| beyond ~1e7 L, NaN, Inf) still
+// lands in a valid cell; k_bin raises the context's non-finite flag for it
 __device__ __forceinline__ int mop_cell1(float xw, float sc, int n) {
     int v = (int)__fmul_rn(xw, sc);
-    return v > n - 1 ? n - 1 : v;
+    v = v > n - 1 ? n - 1 : v;
+    return v < 0 ? 0 : v;
 }
 
-// padding slots sit far outside the box, every slot at its own place (no two dummies coincide)
-__device__ __forceinline__ float4 mop_dummy_xq(int s) {
-    return make_float4(-1000.0f - 4.0f * (float)(s & 1023), -1000.0f - 4.0f * (float)((s >> 10) & 1023),
-                       -1000.0f - 4.0f * (float)(s >> 20), 0.0f);
+// padding slots sit far outside the box on a lattice of three box lengths: slot s -> (a, b, c) = its bit fields,
+// x = -(3a + 2) Lx, y = -(3b + 2) Ly, z = -(3c + 2) Lz.  Two distinct dummies differ by >= 3 L in some component and a
+// real atom (in [0, L)) is >= 2 L away from every dummy, so under any periodic shift (|k| <= 1) no pair that involves
+// a dummy is within r_cut <= L/2: the pair predicate itself rejects them, with finite arithmetic; charge 0, type 0
+__device__ __forceinline__ float4 mop_dummy_xq(int s, const float box[3]) {
+    return make_float4(-(3.0f * (float)(s & 1023) + 2.0f) * box[0], -(3.0f * (float)((s >> 10) & 1023) + 2.0f) * box[1],
+                       -(3.0f * (float)(s >> 20) + 2.0f) * box[2], 0.0f);
 }
 
 __device__ __forceinline__ void mop_red_add_f4(float4 *addr, float x, float y, float z) {

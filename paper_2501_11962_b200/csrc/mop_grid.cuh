@@ -5,16 +5,23 @@
 #pragma once
 #include "mop_common.cuh"
 
-// cell id of every atom + per-cell histogram
+// cell id of every atom + per-cell histogram.  A coordinate that is not finite, or so large that the FP32 wrap cannot
+// bring it into [0, L), raises the sticky non-finite flag (reported as MOP_ERR_NONFINITE at the next synchronising call)
 __global__ void __launch_bounds__(256) k_bin(const float *__restrict__ R, MopGrid g, int *__restrict__ cell,
-                                             int *__restrict__ cell_count) {
+                                             int *__restrict__ cell_count, unsigned *__restrict__ nonfinite) {
     int n = blockIdx.y;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Q) return;
     const float *r = R + ((size_t)n * g.Q + i) * 3;
     int c[3];
+    bool ok = true;
 #pragma unroll
-    for (int d = 0; d < 3; d++) c[d] = mop_cell1(mop_wrap1(r[d], g.box[d], g.inv_box[d]), g.sc[d], g.dims[d]);
+    for (int d = 0; d < 3; d++) {
+        const float xw = mop_wrap1(r[d], g.box[d], g.inv_box[d]);
+        ok = ok && (xw >= 0.0f) && (xw < g.box[d]);   // false for NaN
+        c[d] = mop_cell1(xw, g.sc[d], g.dims[d]);
+    }
+    if (!ok) *nonfinite = 1u;
     int id = (c[0] * g.dims[1] + c[1]) * g.dims[2] + c[2];
     cell[(size_t)n * g.Q + i] = id;
     atomicAdd(&cell_count[(size_t)n * g.ncell + id], 1);
@@ -44,7 +51,7 @@ __global__ void __launch_bounds__(128) k_colscan(MopGrid g, const int *__restric
     if (lane == 0) col_count[(size_t)n * g.ncol + col] = run;
 }
 
-// one CTA per bead: exclusive scan of the column counts rounded up to 32 -> col_start[n][0..ncol]
+// one CTA per bead: exclusive scan of the column counts rounded up to the cluster size -> col_start[n][0..ncol]
 __global__ void __launch_bounds__(1024) k_colstart(MopGrid g, const int *__restrict__ col_count,
                                                    int *__restrict__ col_start) {
     __shared__ int wsum[32];
@@ -55,7 +62,7 @@ __global__ void __launch_bounds__(1024) k_colstart(MopGrid g, const int *__restr
     __syncthreads();
     for (int c0 = 0; c0 < g.ncol; c0 += 1024) {
         int col = c0 + threadIdx.x;
-        int v = col < g.ncol ? ((col_count[(size_t)n * g.ncol + col] + 31) & ~31) : 0;
+        int v = col < g.ncol ? ((col_count[(size_t)n * g.ncol + col] + MOP_CL - 1) & ~(MOP_CL - 1)) : 0;
         int inc = v;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -92,7 +99,7 @@ __global__ void __launch_bounds__(256) k_fill_pad(MopGrid g, int *__restrict__ p
     if (s >= g.S) return;
     size_t o = (size_t)n * g.S + s;
     perm[o] = -1;
-    xq[o] = mop_dummy_xq(s);
+    xq[o] = mop_dummy_xq(s, g.box);
     typ[o] = 0;
 }
 
@@ -137,41 +144,33 @@ __global__ void __launch_bounds__(256) k_rank(const float *__restrict__ R, MopGr
     typ[o] = type_row[i];
 }
 
-// bounding boxes over the real atoms of every j-cluster (32 slots) and of its four i-clusters (8 slots)
+// bounding box over the real atoms of every octet (8 slots); lo.w = number of real atoms (int bits)
 __global__ void __launch_bounds__(128) k_bbox(MopGrid g, const int *__restrict__ perm, const float4 *__restrict__ xq,
-                                              float4 *__restrict__ jlo, float4 *__restrict__ jhi,
-                                              float4 *__restrict__ ilo, float4 *__restrict__ ihi) {
-    int n = blockIdx.y;
-    int cj = blockIdx.x * 4 + (threadIdx.x >> 5);
-    int lane = threadIdx.x & 31;
-    int ncj = g.S / MOP_CJ;
-    if (cj >= ncj) return;
-    size_t o = (size_t)n * g.S + (size_t)cj * MOP_CJ + lane;
-    bool real = perm[o] >= 0;
-    float4 p = xq[o];
+                                              float4 *__restrict__ blo, float4 *__restrict__ bhi) {
+    const int n = blockIdx.y;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;   // S is a multiple of 32: whole warps in range
+    if (s >= g.S) return;
+    const size_t o = (size_t)n * g.S + s;
+    const bool real = perm[o] >= 0;
+    const float4 p = xq[o];
     float lo[3], hi[3];
     const float BIG = 1.0e30f;
     lo[0] = real ? p.x : BIG, lo[1] = real ? p.y : BIG, lo[2] = real ? p.z : BIG;
     hi[0] = real ? p.x : -BIG, hi[1] = real ? p.y : -BIG, hi[2] = real ? p.z : -BIG;
     int cnt = real ? 1 : 0;
 #pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
+    for (int off = 1; off < MOP_CL; off <<= 1) {
 #pragma unroll
         for (int d = 0; d < 3; d++) {
             lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], off));
             hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], off));
         }
         cnt += __shfl_xor_sync(0xffffffffu, cnt, off);
-        if (off == 4 && (lane & 7) == 0) {
-            size_t oi = (size_t)n * (g.S / MOP_CI) + (size_t)cj * 4 + (lane >> 3);
-            ilo[oi] = make_float4(lo[0], lo[1], lo[2], __int_as_float(cnt));
-            ihi[oi] = make_float4(hi[0], hi[1], hi[2], 0.0f);
-        }
     }
-    if (lane == 0) {
-        size_t oj = (size_t)n * ncj + cj;
-        jlo[oj] = make_float4(lo[0], lo[1], lo[2], __int_as_float(cnt));
-        jhi[oj] = make_float4(hi[0], hi[1], hi[2], 0.0f);
+    if ((s & (MOP_CL - 1)) == 0) {
+        const size_t oc = (size_t)n * (g.S / MOP_CL) + s / MOP_CL;
+        blo[oc] = make_float4(lo[0], lo[1], lo[2], __int_as_float(cnt));
+        bhi[oc] = make_float4(hi[0], hi[1], hi[2], 0.0f);
     }
 }
 

@@ -22,8 +22,10 @@ struct NbArgs {
     float4 *out;        // [nf][S] F4 or H4, accumulated with vector reductions
     const MopUnit *units;
     const MopEntry *entries;
-    const unsigned *masks;
+    const unsigned long long *masks; // exclusion rows: byte k = the j slots (bits 0-7) i atom k may interact with
     const MopCounters *ctr;
+    unsigned cap_units;              // units beyond the allocation were never written (overflow): never read them
+    unsigned long long *n_inrange;   // counting variant only: in-range, non-excluded pair decisions of this launch
     unsigned *work;     // dynamic work counter (zeroed before the launch)
     int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all
     const float2 *tab;  // [nt*nt] (6 C6, 12 C12)
@@ -38,7 +40,7 @@ __device__ __forceinline__ float mop_rsqrt(float x) {
     return y;
 }
 
-// G8: the pair predicate.  xs_i = xw_i - k L is formed once per unit (k L exact, one rounding); then
+// G8: the pair predicate.  xs_i = xw_i - k L (k L exact, one rounding; xs_i = xw_i exactly for the zero shift); then
 // d = xs_i - xw_j (one rounding per component), r2 = fma(dz,dz, fma(dy,dy, dx*dx)), in range iff r2 < rc*rc.
 __device__ __forceinline__ float mop_r2(float dx, float dy, float dz) {
     return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
@@ -50,7 +52,7 @@ __device__ __forceinline__ void mop_unit_shift(int s, const float box[3], float 
     sz = (float)(s / 9 - 1) * box[2];
 }
 
-// ---- debug: the set of in-range, non-excluded pairs of one bead, with the force kernel's predicate ----
+// ---- debug: the set of in-range, non-excluded pairs of one bead, scalar restatement of the predicate over the list ----
 struct PairDbgArgs {
     int S, bead;
     float rc2;
@@ -58,41 +60,45 @@ struct PairDbgArgs {
     const int *perm;
     const MopUnit *units;
     const MopEntry *entries;
-    const unsigned *masks;
+    const unsigned long long *masks;
     MopCounters *ctr;
+    unsigned cap_units;
     int *pairs;
     long long cap;
     float box[3];
 };
 
 __global__ void __launch_bounds__(128) k_debug_pairs(const PairDbgArgs a) {
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, g = lane >> 3, jl = lane & 7;
     const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
-    const unsigned nu = a.ctr->n_units;
+    const unsigned nu = min(a.ctr->n_units, a.cap_units);
     for (unsigned u = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); u < nu; u += nwarps) {
         const MopUnit un = a.units[u];
         if (un.bead != a.bead || un.count == 0) continue;
         const float4 *xq = a.xq + (size_t)un.bead * a.S;
         const int *perm = a.perm + (size_t)un.bead * a.S;
-        float sx, sy, sz;
-        mop_unit_shift(un.shift, a.box, sx, sy, sz);
-        for (unsigned e = un.start; e < un.start + un.count; e++) {
-            const MopEntry cur = a.entries[e];
-            const float4 cp = xq[(size_t)cur.x * MOP_CJ + lane];
-            const int pj = perm[(size_t)cur.x * MOP_CJ + lane];
-            const unsigned row1 = cur.y >> 8;
-            for (int k = 0; k < MOP_CI; k++) {
-                if (!((cur.y >> k) & 1u)) continue;
-                const float4 pi = xq[un.ci * MOP_CI + k];
-                bool allowed = true;
-                if (row1) allowed = (a.masks[(size_t)(un.excl_base + row1 - 1) * MOP_CI + k] >> lane) & 1u;
+        for (unsigned e0 = un.start; e0 < un.start + un.count; e0 += MOP_NG) {
+            const MopEntry cur = a.entries[e0 + g];
+            const unsigned pat = cur.y & 15u;
+            if (pat == 0) continue;
+            const unsigned oc = cur.x & 0xffffffu, sid = cur.x >> 24, row1 = cur.y >> 8;
+            float sx, sy, sz;
+            mop_unit_shift((int)sid, a.box, sx, sy, sz);
+            const float4 cp = xq[(size_t)oc * MOP_CL + jl];
+            const int pj = perm[(size_t)oc * MOP_CL + jl];
+            unsigned long long row = ~0ull;
+            if (row1) row = a.masks[(size_t)un.excl_base + row1 - 1];
+            for (int k = 0; k < MOP_CL; k++) {
+                if (!((pat >> (k >> 1)) & 1u)) continue;
+                const float4 pi = xq[un.ci * MOP_CL + k];
+                const bool allowed = (row >> (8 * k + jl)) & 1ull;
                 const float dx = __fsub_rn(__fsub_rn(pi.x, sx), cp.x), dy = __fsub_rn(__fsub_rn(pi.y, sy), cp.y),
                             dz = __fsub_rn(__fsub_rn(pi.z, sz), cp.z);
                 const float r2 = mop_r2(dx, dy, dz);
                 if ((r2 < a.rc2) && allowed) {
                     unsigned long long pos = atomicAdd(&a.ctr->n_pairs, 1ull);
                     if ((long long)pos < a.cap) {
-                        a.pairs[2 * pos] = perm[un.ci * MOP_CI + k];
+                        a.pairs[2 * pos] = perm[un.ci * MOP_CL + k];
                         a.pairs[2 * pos + 1] = pj;
                     }
                 }

@@ -7,8 +7,9 @@
 // Packed variant: two i atoms per lane per issue slot (sm_100a FFMA2 / FMUL2 / FADD2 = fma|mul|add.rn.f32x2).
 // The pair kernels are bound by issue slots when written with scalar FP32 instructions (profiles/r01_ncu_summary.md);
 // the packed form halves the FP issue count, which leaves the FP32 pipe itself (128 lanes/clk/SM) as the bound.
-// Lane l still owns atom l of the current j-cluster; a packed register holds the same quantity for i atoms
-// (2p, 2p+1), p = 0..3.  All packed operations are IEEE round-to-nearest per component, so the G8 predicate
+// Lane (jl = lane & 7, g = lane >> 3) owns atom jl of the g-th of the four j-octets of the current step; a packed
+// register holds the same quantity for i atoms (2p, 2p+1), p = 0..3.  All packed operations are IEEE
+// round-to-nearest per component, so the G8 predicate
 // (d = xs_i - xw_j, r2 = fma(dz,dz,fma(dy,dy,dx*dx)), r2 < rc*rc) is bit-identical to the scalar form.
 // Sign conventions chosen so that no negation is needed in the row body:
 //   gn = -g = x (B - A) + C - 2 k_rf ke qi qj,      hn = -h = x (x (8A - 14B) - 3C),      dn = s_j - s_i = -delta
@@ -88,14 +89,12 @@ __device__ __forceinline__ void mop_cp_wait() {
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
-       NBP_OCC6 = 4 };  // ask for 6 resident CTAs per SM (register cap 80)
-#define NBP_NST 2       // stages of the per-warp j-atom ring (entries in flight: NBP_NST - 1; 2 measured best of 2, 3, 4, 6)
+#define NBP_NST 2       // stages of the per-warp j-atom ring (steps in flight: NBP_NST - 1)
 
 // Shared memory of one CTA (4 warps), bytes:
 //   [0, 1024)              i-atom staging, 256 B per warp: for p = 0..3 at float offset 16 p
 //                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
-//   [1024, 2048)           the current chunk of up to 32 list entries, 256 B per warp
+//   [1024, 2048)           the current chunk of up to 32 list entries (8 steps), 256 B per warp
 //   [2048, 2048 + 4 NBP_NST KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
 //   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), energy shift [nt*nt],
 //   and one flag per type: its LJ row has a non-zero entry
@@ -104,11 +103,15 @@ enum { NBP_OCC5 = 2,    // ask for 5 resident CTAs per SM (register cap 96)
 #define NBP_SM_TAB (2048u + 4u * NBP_NST * 1024u)
 __host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 12 + (size_t)nt * 4; }
 
-template <int MODE, int VAR>
+// One work unit = one i-octet against its list of (j-octet, shift) entries, four entries per step: lane (jl, g) holds
+// atom jl of the step's g-th octet.  The builder has ordered the entries by their row-pair pattern, so the union
+// pattern of a step (which row pairs the warp evaluates) mostly equals each group's own.  A group whose own pattern
+// lacks a row pair of the union evaluates it too; its pairs are out of range there by construction of the pattern
+// (the builder's test is a superset of G8), so the exact per-pair predicate masks them.
+template <int MODE, bool COUNT>
 __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, float *__restrict__ sw,
                                          const unsigned sw_addr, const unsigned se_addr, const unsigned sr_addr,
                                          const unsigned tab6, const unsigned off12,
-                                         const float *__restrict__ tabs,
                                          const int *__restrict__ tflag, const int lane) {
     constexpr bool HVP = MODE == NB_HVP, ENERGY = MODE == NB_ENERGY;
     const unsigned boff = (unsigned)un.bead * (unsigned)a.S; // nf * S < 2^31 (checked at create)
@@ -116,24 +119,23 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     const float4 *__restrict__ et = a.et + boff;
     const int *__restrict__ typ = a.typ + boff;
     float4 *__restrict__ out = a.out + boff;
+    const int jl = lane & 7, gq = lane >> 3;
 
     __syncwarp();
     bool has_lj = false;
-    if (lane < MOP_CI) {
-        float sx, sy, sz;
-        mop_unit_shift(un.shift, a.box, sx, sy, sz);
-        float4 p = xq[un.ci * MOP_CI + lane];
+    if (lane < MOP_CL) {
+        float4 p = xq[un.ci * MOP_CL + lane];
         float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
         int ti;
         if (HVP) {
-            e = et[un.ci * MOP_CI + lane];
+            e = et[un.ci * MOP_CL + lane];
             ti = __float_as_int(e.w);
         } else {
-            ti = typ[un.ci * MOP_CI + lane];
+            ti = typ[un.ci * MOP_CL + lane];
         }
         has_lj = tflag[ti] != 0;
         float *d = sw + (lane >> 1) * 16 + (lane & 1);
-        d[0] = __fsub_rn(p.x, sx), d[2] = __fsub_rn(p.y, sy), d[4] = __fsub_rn(p.z, sz);
+        d[0] = p.x, d[2] = p.y, d[4] = p.z;
         d[6] = p.w * MOP_KE;
         d[8] = e.x, d[10] = e.y, d[12] = e.z;
         d[14] = __int_as_float((int)tab6 + ti * a.nt * 4);
@@ -145,46 +147,54 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
 #pragma unroll
     for (int p = 0; p < 4; p++) ax[p] = ay[p] = az[p] = 0ull;
     double e_lj = 0.0, e_c = 0.0;
+    unsigned n_in = 0;
     const f2 nk2rf = f2_bc(-a.k2rf);
     const unsigned lane16 = (unsigned)lane * 16u;
 
-    // one entry: the 32 j atoms (cp, ce, type offset tj4) against the 8 i atoms.
-    // Phase L (branch-free, four independent chains): d, r2 and the G8 test for all four packed row pairs.
-    // Phase H: the pair math for the row pairs in which some lane is in range (warp votes).
-    auto entry = [&](const uint2 cur, const float4 cp, const float4 ce, const unsigned tj4) {
+    // one step: the lane's j atom (cp, ce, type offset tj4) against the row pairs of the union pattern `upat`.
+    // sh*: the lane's periodic shift (packed broadcast; zero for most steps: x - 0 = x exactly, so one code path
+    // serves both, the shifted form only being compiled into the SHIFTED instance).
+    auto step = [&](const uint2 cur, const unsigned upat, const bool shifted, const float4 cp, const float4 ce,
+                    const unsigned tj4) {
         const f2 jx = f2_bc(cp.x), jy = f2_bc(cp.y), jz = f2_bc(cp.z), jq = f2_bc(cp.w);
-        f2 r2v[4];
-        bool anyp[4];
-#pragma unroll
-        for (int p = 0; p < 4; p++) {
-            const float4 P0 = mop_lds_v4(sw_addr + p * 64);
-            const float2 P1 = mop_lds_v2(sw_addr + p * 64 + 16);
-            const f2 dx = f2_sub(f2_pack(P0.x, P0.y), jx), dy = f2_sub(f2_pack(P0.z, P0.w), jy),
-                     dz = f2_sub(f2_pack(P1.x, P1.y), jz);
-            r2v[p] = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
-            float r2a, r2b;
-            f2_unpack(r2v[p], r2a, r2b);
-            anyp[p] = __any_sync(0xffffffffu, fminf(r2a, r2b) < a.rc2);
+        f2 shx = 0ull, shy = 0ull, shz = 0ull;
+        if (shifted) {
+            float sx, sy, sz;
+            mop_unit_shift((int)(cur.x >> 24), a.box, sx, sy, sz);
+            shx = f2_bc(sx), shy = f2_bc(sy), shz = f2_bc(sz);
         }
-        if (!(anyp[0] || anyp[1] || anyp[2] || anyp[3])) return;
         f2 nx = 0ull, ny = 0ull, nz = 0ull; // jn: minus the j-side sums
         float u_lj = 0.f, u_c = 0.f;
+        // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
+        // (a padding entry -- pattern 0, it points at the unit's own octet -- allows nothing)
+        const bool valid = (cur.y & 15u) != 0u;
+        unsigned lm = valid ? 0xffu : 0u;
+        const unsigned row1 = cur.y >> 8;
+        const bool masked = __any_sync(0xffffffffu, row1 != 0 || !valid);
+        if (masked && row1 != 0) {
+            const unsigned long long row = a.masks[(size_t)un.excl_base + row1 - 1];
+            const unsigned w0 = ((unsigned)row >> jl) & 0x01010101u, w1 = ((unsigned)(row >> 32) >> jl) & 0x01010101u;
+            lm = ((w0 | (w0 >> 7) | (w0 >> 14) | (w0 >> 21)) & 0xfu) | (((w1 | (w1 >> 7) | (w1 >> 14) | (w1 >> 21)) & 0xfu) << 4);
+        }
 
-        auto heavy = [&](const int p, const bool masked, const unsigned lm, const bool nolj) {
+        auto heavy = [&](const int p, const bool nolj) {
             const float4 P0 = mop_lds_v4(sw_addr + p * 64), P1 = mop_lds_v4(sw_addr + p * 64 + 16);
-            const f2 dx = f2_sub(f2_pack(P0.x, P0.y), jx), dy = f2_sub(f2_pack(P0.z, P0.w), jy),
-                     dz = f2_sub(f2_pack(P1.x, P1.y), jz), Qi = f2_pack(P1.z, P1.w);
+            f2 X = f2_pack(P0.x, P0.y), Y = f2_pack(P0.z, P0.w), Z = f2_pack(P1.x, P1.y);
+            if (shifted) X = f2_sub(X, shx), Y = f2_sub(Y, shy), Z = f2_sub(Z, shz);
+            const f2 dx = f2_sub(X, jx), dy = f2_sub(Y, jy), dz = f2_sub(Z, jz), Qi = f2_pack(P1.z, P1.w);
+            const f2 r2v = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
             float r2a, r2b;
-            f2_unpack(r2v[p], r2a, r2b);
-            bool ina = r2a < a.rc2, inb = r2b < a.rc2; // G8
+            f2_unpack(r2v, r2a, r2b);
+            bool ina = r2a < a.rc2, inb = r2b < a.rc2; // G8 (padding atoms are never in range: mop_dummy_xq)
             if (masked) {
                 ina = ina && ((lm >> (2 * p)) & 1u);
                 inb = inb && ((lm >> (2 * p + 1)) & 1u);
             }
+            if (COUNT) n_in += (ina ? 1u : 0u) + (inb ? 1u : 0u);
             const float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
             f2 rinv = f2_pack(ra, rb);
             if (ENERGY) { // one Newton step: removes the approximation's bias from the energy sum
-                const f2 em = f2_fma(f2_mul(r2v[p], rinv), rinv, f2_bc(-1.0f));   // r2 rinv^2 - 1
+                const f2 em = f2_fma(f2_mul(r2v, rinv), rinv, f2_bc(-1.0f));   // r2 rinv^2 - 1
                 rinv = f2_fma(f2_mul(rinv, f2_bc(-0.5f)), em, rinv);
             }
             f2 S0 = 0ull, S1 = 0ull, S2 = 0ull;
@@ -220,7 +230,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 f2_acc(ax[p], gn, dx), f2_acc(ay[p], gn, dy), f2_acc(az[p], gn, dz);
                 f2_acc(nx, gn, dx), f2_acc(ny, gn, dy), f2_acc(nz, gn, dz);
                 if (ENERGY) { // u_lj = C12 x^6 - C6 x^3 - shift = B/12 - A/6 - shift;  u_c = ke qi qj (1/r + k_rf r^2 - c_rf)
-                    f2 ue = f2_mul(qq, f2_add(f2_fma(r2v[p], f2_bc(a.krf), rinv), f2_bc(-a.crf)));
+                    f2 ue = f2_mul(qq, f2_add(f2_fma(r2v, f2_bc(a.krf), rinv), f2_bc(-a.crf)));
                     if (!nolj) {
                         const f2 sh = f2_pack(mop_lds_f(ta + 2u * off12), mop_lds_f(tb + 2u * off12));
                         const f2 ul = f2_fma(B, f2_bc(1.0f / 12.0f), f2_fma(A, f2_bc(-1.0f / 6.0f), f2_mul(sh, f2_bc(-1.0f))));
@@ -251,53 +261,36 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             }
         };
 
-        const unsigned row1 = cur.y >> 8;
-        if (row1 == 0) { // no exclusions in this cluster pair
 #pragma unroll
-            for (int p = 0; p < 4; p++)
-                if (anyp[p]) {
-                    if ((ljmask >> (2 * p)) & 3u) heavy(p, false, 0u, false);
-                    else heavy(p, false, 0u, true);
-                }
-        } else { // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
-            const uint4 *__restrict__ mrow =
-                reinterpret_cast<const uint4 *>(a.masks + (size_t)(un.excl_base + row1 - 1) * MOP_CI);
-            const uint4 m0 = mrow[0], m1 = mrow[1];
-            const unsigned mm[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
-            unsigned lm = 0;
-#pragma unroll
-            for (int k = 0; k < MOP_CI; k++) lm |= ((mm[k] >> lane) & 1u) << k;
-#pragma unroll
-            for (int p = 0; p < 4; p++)
-                if (anyp[p]) {
-                    if ((ljmask >> (2 * p)) & 3u) heavy(p, true, lm, false);
-                    else heavy(p, true, lm, true);
-                }
-        }
-        {
+        for (int p = 0; p < 4; p++)
+            if ((upat >> p) & 1u) {
+                if ((ljmask >> (2 * p)) & 3u) heavy(p, false);
+                else heavy(p, true);
+            }
+        if (valid) {
             float lx, hx, ly, hy, lz, hz;
             f2_unpack(nx, lx, hx), f2_unpack(ny, ly, hy), f2_unpack(nz, lz, hz);
-            mop_red_add_f4(out + (cur.x * MOP_CJ + lane), -lx - hx, -ly - hy, -lz - hz);
+            mop_red_add_f4(out + ((cur.x & 0xffffffu) * MOP_CL + jl), -lx - hx, -ly - hy, -lz - hz);
         }
         if (ENERGY) e_lj += (double)u_lj, e_c += (double)u_c;
     };
 
-    // ---- the unit's entries, 32 at a time: the chunk's entry words go to shared memory (one coalesced load), the
-    // j atoms of the next NBP_NST-1 entries are in flight (cp.async into the warp's ring; every lane copies and
+    // ---- the unit's entries, 32 at a time (8 steps): the chunk's entry words go to shared memory (one coalesced load),
+    // the j atoms of the next NBP_NST-1 steps are in flight (cp.async into the warp's ring; every lane copies and
     // later reads only its own atom, so no cross-lane synchronisation is needed)
     const unsigned eend = un.start + un.count;
     for (unsigned c0 = un.start; c0 < eend; c0 += 32) {
-        const int nE = (int)min(32u, eend - c0);
+        const int nE = (int)min(32u, eend - c0), nS = nE / MOP_NG;
         __syncwarp();
         if (lane < nE) {
             const uint2 w = a.entries[c0 + lane];
             asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(se_addr + lane * 8), "r"(w.x), "r"(w.y) : "memory");
         }
         __syncwarp();
-        auto issue = [&](const int k) { // start the copies of entry k's j atoms into stage k % NBP_NST
-            if (k < nE) {
-                const unsigned jc = mop_lds_vu(se_addr + k * 8);
-                const unsigned o = jc * MOP_CJ + lane;
+        auto issue = [&](const int k) { // start the copies of step k's j atoms into stage k % NBP_NST
+            if (k < nS) {
+                const unsigned jc = mop_lds_vu(se_addr + (k * MOP_NG + gq) * 8) & 0xffffffu;
+                const unsigned o = jc * MOP_CL + jl;
                 const unsigned st = sr_addr + (unsigned)(k % NBP_NST) * 1024u;
                 mop_cp_async16(st + lane16, xq + o);
                 if (HVP) mop_cp_async16(st + 512u + lane16, et + o);
@@ -307,11 +300,11 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         };
 #pragma unroll
         for (int k = 0; k < NBP_NST - 1; k++) issue(k);
-        for (int i = 0; i < nE; i++) {
+        for (int i = 0; i < nS; i++) {
             issue(i + NBP_NST - 1);
             mop_cp_wait<NBP_NST - 1>();
             const unsigned st = sr_addr + (unsigned)(i % NBP_NST) * 1024u;
-            const uint2 cur = mop_lds_vu2(se_addr + i * 8);
+            const uint2 cur = mop_lds_vu2(se_addr + (i * MOP_NG + gq) * 8);
             const float4 cp = mop_lds_v4(st + lane16);
             float4 ce = make_float4(0.f, 0.f, 0.f, 0.f);
             unsigned tj4;
@@ -321,7 +314,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             } else {
                 tj4 = mop_lds_vu(st + 512u + lane * 4) * 4u;
             }
-            entry(cur, cp, ce, tj4);
+            const unsigned upat = __reduce_or_sync(0xffffffffu, cur.y & 15u);
+            const bool shifted = __any_sync(0xffffffffu, (cur.x >> 24) != MOP_NOSHIFT);
+            if (shifted) step(cur, upat, true, cp, ce, tj4);
+            else step(cur, upat, false, cp, ce, tj4);
         }
         mop_cp_wait<0>();
     }
@@ -349,7 +345,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         v[j] += __shfl_xor_sync(0xffffffffu, v[j], 2);
         v[j] += __shfl_xor_sync(0xffffffffu, v[j], 1);
     }
-    if ((lane & 3) == 0) mop_red_add_f4(out + (un.ci * MOP_CI + (lane >> 2)), v[0], v[1], v[2]);
+    if ((lane & 3) == 0) mop_red_add_f4(out + (un.ci * MOP_CL + (lane >> 2)), v[0], v[1], v[2]);
     if (ENERGY) {
         e_lj = mop_warp_sum_d(e_lj), e_c = mop_warp_sum_d(e_c);
         if (lane == 0) {
@@ -357,10 +353,15 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             atomicAdd(&a.energies[1], e_c);
         }
     }
+    if (COUNT) {
+        n_in = (unsigned)__reduce_add_sync(0xffffffffu, n_in);
+        if (lane == 0) atomicAdd(a.n_inrange, (unsigned long long)n_in);
+    }
 }
 
-template <int MODE, int VAR>
-__global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ? 5 : 4) k_nonbonded_p(const NbArgs a) {
+// persistent grid (resident CTAs x SMs) with a dynamic work counter; CTAS = resident CTAs per SM asked for
+template <int MODE, bool COUNT, int CTAS>
+__global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
     extern __shared__ float4 s_dyn[];
     char *sb = reinterpret_cast<char *>(s_dyn);
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -380,9 +381,10 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
         tflag[t] = f;
     }
     __syncthreads();
-    unsigned ubeg = 0, uend = a.ctr->n_units;
-    if (a.range == 0) uend = a.ctr->n_units_bead0;
-    else if (a.range == 1) ubeg = a.ctr->n_units_bead0;
+    const unsigned nu = min(a.ctr->n_units, a.cap_units), nu0 = min(a.ctr->n_units_bead0, a.cap_units);
+    unsigned ubeg = 0, uend = nu;
+    if (a.range == 0) uend = nu0;
+    else if (a.range == 1) ubeg = nu0;
     const unsigned s0 = (unsigned)__cvta_generic_to_shared(sb);
     const unsigned sw_addr = s0 + w * 256u, se_addr = s0 + NBP_SM_ENT + w * 256u;
     const unsigned sr_addr = s0 + NBP_SM_RING + w * (NBP_NST * 1024u);
@@ -395,9 +397,9 @@ __global__ void __launch_bounds__(128, (VAR & NBP_OCC6) ? 6 : (VAR & NBP_OCC5) ?
         const uint4 *up = reinterpret_cast<const uint4 *>(a.units + u);
         const uint4 u0 = up[0], u1 = up[1];
         MopUnit un;
-        un.bead = (int)u0.x, un.ci = (int)u0.y, un.shift = (int)u0.z, un.start = u0.w;
-        un.count = u1.x, un.excl_base = u1.y;
+        un.bead = (int)u0.x, un.ci = (int)u0.y, un.start = u0.z, un.count = u0.w;
+        un.excl_base = u1.x;
         if (un.count == 0) continue;
-        nbp_unit<MODE, VAR>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tabs, tflag, lane);
+        nbp_unit<MODE, COUNT>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tflag, lane);
     }
 }

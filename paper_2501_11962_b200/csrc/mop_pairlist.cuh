@@ -1,27 +1,31 @@
-// mop_pairlist.cuh -- S1: cluster-pair list.
+// mop_pairlist.cuh -- S1: octet-pair list with exact row-pair patterns.
 //
-// One warp per i-cluster (8 consecutive sorted slots).  For every periodic shift it lists the j-clusters
-// (32 slots, index >= the i-cluster's own j-cluster: half list) whose bounding box comes within r_list of the
-// i-cluster's box, with an 8-bit mask of the i atoms that come within r_list of the j box, and the index of
-// an exclusion-mask row when the cluster pair holds excluded pairs (or is the diagonal block, where only
-// lane > own lane is allowed).  Output: work units (bead, i-cluster, shift) -> contiguous entry ranges.
+// One warp per i-octet (8 consecutive sorted slots).  It lists every (j-octet, periodic shift) with j-octet index
+// >= its own (half list) in which some atom pair comes within r_list, together with
+//   - a 4-bit pattern: row pair p (i atoms 2p, 2p+1) has such a pair (evaluated atom by atom with the FP32 form of
+//     the pair kernels' distance, against r_list^2 inflated by 1e-4: a superset of what the kernels accept),
+//   - the index of an exclusion-mask row when the octet pair holds excluded pairs (or is the diagonal block, where
+//     only j slot > i slot is allowed).
+// The entries of a unit are written ordered by pattern, so that the four octets a warp of the pair kernels takes per
+// step mostly share theirs, and padded to a multiple of four with pattern-0 entries.
 // The list is only a superset; the pair kernels apply the exact FP32 predicate (G8) per atom pair.
 #pragma once
 #include "mop_common.cuh"
+#include "mop_nonbonded.cuh"
 
 struct PlArgs {
     MopGrid g;
     int bead0;
     float rl, rl2; // list radius, and its square inflated by 1e-4 (conservative against FP32 rounding)
     const int *perm, *slot_of;
-    const float4 *xq, *jlo, *jhi, *ilo, *ihi;
+    const float4 *xq, *blo, *bhi;
     const int *col_start, *cell_rel, *col_count;
     const int *excl_start, *excl_list; // may be NULL
     MopUnit *units;
     MopEntry *entries;
-    unsigned *masks;
+    unsigned long long *masks;
     MopCounters *ctr;
-    unsigned long long *slots_active; // sum over entries of popc(imask)
+    unsigned long long *slots_active; // sum over entries of popc(pattern) * 16
     unsigned cap_units, cap_entries, cap_masks;
 };
 
@@ -30,55 +34,64 @@ __device__ __forceinline__ float mop_gap(float lo_a, float hi_a, float lo_b, flo
     return fmaxf(0.0f, fmaxf(lo_b - hi_a, lo_a - hi_b));
 }
 
+// bucket order of the 15 non-zero patterns: full first, then the contiguous runs (the usual partial patterns, the
+// row pairs of an octet being ordered along z), then the rest
+__constant__ unsigned char c_pat_order[16] = {15, 7, 3, 1, 14, 12, 8, 6, 2, 4, 5, 9, 10, 11, 13, 0};
+
 __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
-    __shared__ float4 s_ia[4][MOP_CI];
     __shared__ int s_exJ[4][MOP_EXROWS];
-    __shared__ unsigned s_exM[4][MOP_EXROWS][MOP_CI];
+    __shared__ unsigned s_exM[4][MOP_EXROWS][2];
     __shared__ int s_exN[4];
-    __shared__ int s_bcj[4][MOP_LBUF];
+    __shared__ unsigned s_bcj[4][MOP_LBUF];
     __shared__ unsigned s_binfo[4][MOP_LBUF];
+    __shared__ unsigned s_pcnt[4][16];
 
     const MopGrid &g = a.g;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = a.bead0 + blockIdx.y;
     const int ci = blockIdx.x * 4 + w;
-    const int nci = g.S / MOP_CI, ncj = g.S / MOP_CJ;
-    if (ci >= nci) return;
-    const float4 blo = a.ilo[(size_t)n * nci + ci], bhi = a.ihi[(size_t)n * nci + ci];
-    if (__float_as_int(blo.w) == 0) return; // no real atom in this i-cluster
+    const int noc = g.S / MOP_CL;
+    if (ci >= noc) return;
+    const float4 blo = a.blo[(size_t)n * noc + ci], bhi = a.bhi[(size_t)n * noc + ci];
+    if (__float_as_int(blo.w) == 0) return; // no real atom in this octet
 
     const int *perm = a.perm + (size_t)n * g.S;
     const int *slot_of = a.slot_of + (size_t)n * g.Q;
     const float4 *xq = a.xq + (size_t)n * g.S;
-    const float4 *jlo = a.jlo + (size_t)n * ncj, *jhi = a.jhi + (size_t)n * ncj;
+    const float4 *jlo = a.blo + (size_t)n * noc, *jhi = a.bhi + (size_t)n * noc;
     const int *col_start = a.col_start + (size_t)n * (g.ncol + 1);
-    float4 *ia = s_ia[w];
     int *exJ = s_exJ[w];
-    unsigned(*exM)[MOP_CI] = s_exM[w];
-    int *bcj = s_bcj[w];
-    unsigned *binfo = s_binfo[w];
-    const int J0 = ci >> 2;
+    unsigned(*exM)[2] = s_exM[w];
+    unsigned *bcj = s_bcj[w], *binfo = s_binfo[w], *pcnt = s_pcnt[w];
+    const int J0 = ci;
 
-    if (lane < MOP_CI) {
-        int s = ci * MOP_CI + lane;
-        float4 p = xq[s];
-        p.w = perm[s] >= 0 ? 1.0f : 0.0f;
-        ia[lane] = p;
-        int li = (ci & 3) * MOP_CI + lane; // own lane inside the diagonal j-cluster: only lanes > li are allowed
-        exM[0][lane] = li == 31 ? 0u : (0xffffffffu << (li + 1));
+    if (lane < MOP_EXROWS) {
+        // row 0: the octet itself, only j slot > i slot (byte k of the 64-bit row = allowed j slots of i atom k)
+        unsigned lo = 0, hi = 0;
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                lo |= ((0xffu << (k + 1)) & 0xffu) << (8 * k);
+                hi |= ((0xffu << (k + 5)) & 0xffu) << (8 * k);
+            }
+        }
+        exM[lane][0] = lane == 0 ? lo : 0xffffffffu;
+        exM[lane][1] = lane == 0 ? hi : 0xffffffffu;
     }
+    for (int t = 32 + lane; t < MOP_EXROWS; t += 32) exM[t][0] = exM[t][1] = 0xffffffffu;
+    if (lane < 16) pcnt[lane] = 0;
     if (lane == 0) {
         exJ[0] = J0;
         s_exN[w] = 1;
     }
     __syncwarp();
 
-    // ---- exclusion rows: for each i atom, clear the bit of every excluded partner in its j-cluster's row
+    // ---- exclusion rows: for each i atom, clear the bit of every excluded partner in its j-octet's row
     // (four lanes per i atom, so the dependent loads perm -> excl_start -> excl_list -> slot_of of the 8 atoms are
     // in flight together instead of one atom after the other)
     if (a.excl_start != nullptr) {
         const int k = lane >> 2, sub = lane & 3;
-        const int orig = perm[ci * MOP_CI + k];
+        const int orig = perm[ci * MOP_CL + k];
         int e0 = 0, e1 = 0;
         if (orig >= 0) e0 = a.excl_start[orig], e1 = a.excl_start[orig + 1];
         const int maxn = __reduce_max_sync(0xffffffffu, e1 - e0);
@@ -88,8 +101,8 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
             int J = -1, bit = 0;
             if (act) {
                 const int ps = slot_of[a.excl_list[e]];
-                J = ps >> 5;
-                bit = ps & 31;
+                J = ps >> 3;
+                bit = ps & 7;
                 if (J < J0) act = false; // never listed from this side
             }
             unsigned pend = __ballot_sync(0xffffffffu, act);
@@ -97,24 +110,26 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
                 const int leader = __ffs(pend) - 1;
                 const int Jl = __shfl_sync(0xffffffffu, J, leader);
                 const int nrow = s_exN[w];
-                const unsigned hit = __ballot_sync(0xffffffffu, lane < nrow && exJ[lane] == Jl);
-                int row;
-                if (hit) {
-                    row = __ffs(hit) - 1;
-                } else if (nrow < MOP_EXROWS) {
-                    row = nrow;
-                    if (lane == 0) {
-                        exJ[nrow] = Jl;
-                        s_exN[w] = nrow + 1;
+                unsigned hit = __ballot_sync(0xffffffffu, lane < nrow && exJ[lane] == Jl);
+                int row = hit ? __ffs(hit) - 1 : -1;
+                if (!hit && nrow > 32) {
+                    hit = __ballot_sync(0xffffffffu, lane + 32 < nrow && exJ[lane + 32] == Jl);
+                    if (hit) row = 32 + __ffs(hit) - 1;
+                }
+                if (row < 0) {
+                    if (nrow < MOP_EXROWS) {
+                        row = nrow;
+                        if (lane == 0) {
+                            exJ[nrow] = Jl;
+                            s_exN[w] = nrow + 1;
+                        }
+                    } else if (lane == 0) {
+                        atomicOr(&a.ctr->overflow, 16u);
                     }
-                    if (lane < MOP_CI) exM[nrow][lane] = 0xffffffffu;
-                } else {
-                    row = -1;
-                    if (lane == 0) atomicOr(&a.ctr->overflow, 16u);
                 }
                 __syncwarp();
                 const bool same = act && J == Jl;
-                if (same && row >= 0) atomicAnd(&exM[row][k], ~(1u << bit));
+                if (same && row >= 0) atomicAnd(&exM[row][k >> 2], ~(1u << (8 * (k & 3) + bit)));
                 pend &= ~__ballot_sync(0xffffffffu, same);
                 __syncwarp();
             }
@@ -123,10 +138,10 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
     __syncwarp();
     const int exN = s_exN[w];
 
-    // ---- phase 1: candidate j-clusters.  Each lane takes one neighbouring column (under its x,y periodic image)
+    // ---- phase 1: candidate j-octets.  Each lane takes one neighbouring column (under its x,y periodic image)
     // and one z image; the column's z bins (S0's thin cells) give the slot range that can hold atoms within
-    // r_list in z, hence a short run of j-clusters.  The runs of the 32 lanes are enumerated flat (prefix sum +
-    // binary search), so every lane tests one cluster bounding box per iteration.
+    // r_list in z, hence a short run of octets.  The runs of the 32 lanes are enumerated flat (prefix sum +
+    // binary search), so every lane tests one octet bounding box per iteration.
     const int nx = g.dims[0], ny = g.dims[1], nz = g.dims[2];
     const int cx = mop_cell1(blo.x, g.sc[0], nx), cy = mop_cell1(blo.y, g.sc[1], ny);
     const int mx = (int)floorf(a.rl / g.colw[0]) + 1, my = (int)floorf(a.rl / g.colw[1]) + 1;
@@ -162,8 +177,8 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
                         const int r0 = cell_rel[(size_t)col * nz + b0];
                         const int r1 = b1 + 1 < nz ? cell_rel[(size_t)col * nz + b1 + 1] : col_count[col];
                         if (r1 > r0) {
-                            first = max((s0 + r0) >> 5, J0); // half list: never below the own j-cluster
-                            cnt = max(((s0 + r1 - 1) >> 5) - first + 1, 0);
+                            first = max((s0 + r0) >> 3, J0); // half list: never below the own octet
+                            cnt = max(((s0 + r1 - 1) >> 3) - first + 1, 0);
                             sid = (unsigned)((kx + 1) + 3 * (ky + 1) + 9 * (kz + 1));
                         }
                     }
@@ -205,10 +220,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
                 const unsigned bal = __ballot_sync(0xffffffffu, ok);
                 if (ok) {
                     const int pos = nbuf + __popc(bal & ((1u << lane) - 1));
-                    if (pos < MOP_LBUF) {
-                        bcj[pos] = cj;
-                        binfo[pos] = s_sid;
-                    }
+                    if (pos < MOP_LBUF) bcj[pos] = (unsigned)cj | (s_sid << 24);
                 }
                 nbuf += __popc(bal);
             }
@@ -219,102 +231,117 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         if (lane == 0) atomicOr(&a.ctr->overflow, 8u);
         nbuf = MOP_LBUF;
     }
-    // ---- phase 2: per candidate, which i atoms come within r_list of the j box (imask), and the exclusion row
-    unsigned shift_seen = 0;
-    unsigned nslots = 0;
-    for (int b = 0; b < nbuf; b += 32) {
-        const int idx = b + lane;
-        unsigned info = 0xffffffffu; // dead
-        if (idx < nbuf) {
-            const int cj = bcj[idx];
-            const unsigned sid = binfo[idx];
-            float4 lo = jlo[cj], hi = jhi[cj];
-            float sx, sy, sz;
-            mop_unit_shift((int)sid, g.box, sx, sy, sz);
-            lo.x += sx, hi.x += sx, lo.y += sy, hi.y += sy, lo.z += sz, hi.z += sz;
-            unsigned imask = 0;
+
+    // ---- phase 2: four candidates per step, lane = (j atom jl, candidate g): the 8 i atoms against the lane's j atom
+    // with the arithmetic of the pair kernels (xs_i = x_i - k L, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx)));
+    // pattern bit p = some pair of row pair p within r_list.  Padding atoms are never within range (mop_dummy_xq).
+    const int gq = lane >> 3, jl = lane & 7;
+    float xi[MOP_CL], yi[MOP_CL], zi[MOP_CL];
 #pragma unroll
-            for (int k = 0; k < MOP_CI; k++) {
-                const float4 p = ia[k];
-                const float px = mop_gap(p.x, p.x, lo.x, hi.x), py = mop_gap(p.y, p.y, lo.y, hi.y),
-                            pz = mop_gap(p.z, p.z, lo.z, hi.z);
-                if (p.w != 0.0f && px * px + py * py + pz * pz < a.rl2) imask |= 1u << k;
+    for (int k = 0; k < MOP_CL; k++) {
+        const float4 p = xq[ci * MOP_CL + k];
+        xi[k] = p.x, yi[k] = p.y, zi[k] = p.z;
+    }
+    unsigned nslots = 0;
+    for (int b = 0; b < nbuf; b += MOP_NG) {
+        const int idx = b + gq;
+        const bool live = idx < nbuf;
+        const unsigned cw = live ? bcj[idx] : ((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24));
+        const int cj = (int)(cw & 0xffffffu);
+        const unsigned sid = cw >> 24;
+        const float4 pj = xq[cj * MOP_CL + jl];
+        float sx, sy, sz;
+        mop_unit_shift((int)sid, g.box, sx, sy, sz);
+        unsigned pat = 0;
+#pragma unroll
+        for (int p = 0; p < 4; p++) {
+            bool in = false;
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int k = 2 * p + h;
+                const float dx = __fsub_rn(__fsub_rn(xi[k], sx), pj.x), dy = __fsub_rn(__fsub_rn(yi[k], sy), pj.y),
+                            dz = __fsub_rn(__fsub_rn(zi[k], sz), pj.z);
+                in = in || (mop_r2(dx, dy, dz) < a.rl2);
             }
-            if (imask != 0) {
-                unsigned row1 = 0;
-                for (int t = 0; t < exN; t++)
-                    if (exJ[t] == cj) row1 = (unsigned)t + 1;
-                info = imask | (row1 << 8) | (sid << 16);
-                nslots += __popc(imask);
+            const unsigned bal = __ballot_sync(0xffffffffu, in && live);
+            if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
+        }
+        // exclusion row of this octet pair (at most one row matches)
+        unsigned row1 = 0;
+        for (int t0 = 0; t0 < exN; t0 += 8) {
+            const bool hit = pat != 0 && t0 + jl < exN && exJ[t0 + jl] == cj;
+            const unsigned hb = (__ballot_sync(0xffffffffu, hit) >> (8 * gq)) & 0xffu;
+            if (hb) row1 = (unsigned)(t0 + __ffs(hb));
+        }
+        if (live && jl == 0) {
+            unsigned info = 0;
+            if (pat != 0) {
+                const unsigned pos = atomicAdd(&pcnt[pat], 1u);
+                info = pat | (row1 << 8) | (pos << 16);
+                nslots += __popc(pat) * 16u;
             }
             binfo[idx] = info;
         }
-        // the shifts that occur among the live candidates of this batch
-        unsigned live = __ballot_sync(0xffffffffu, info != 0xffffffffu);
-        while (live) {
-            const int l = __ffs(live) - 1;
-            const unsigned sidl = __shfl_sync(0xffffffffu, info, l) >> 16;
-            shift_seen |= 1u << sidl;
-            live &= ~__ballot_sync(0xffffffffu, info != 0xffffffffu && (info >> 16) == sidl);
-        }
     }
     __syncwarp();
-    if (shift_seen == 0) return;
-    nslots = (unsigned)__reduce_add_sync(0xffffffffu, nslots);
-    if (lane == 0) atomicAdd(a.slots_active, (unsigned long long)nslots);
 
-    // ---- exclusion-mask rows of this i-cluster
-    unsigned mb = 0;
-    if (lane == 0) mb = atomicAdd(&a.ctr->n_masks, (unsigned)exN);
-    mb = __shfl_sync(0xffffffffu, mb, 0);
-    if (mb + exN > a.cap_masks) {
-        if (lane == 0) atomicOr(&a.ctr->overflow, 4u);
-        return;
+    // ---- bucket starts in pattern order, total, padded total
+    unsigned mycnt = 0, mypat = 0;
+    if (lane < 15) {
+        mypat = c_pat_order[lane];
+        mycnt = pcnt[mypat];
     }
-    for (int t = lane; t < exN * MOP_CI; t += 32) a.masks[(size_t)mb * MOP_CI + t] = exM[t / MOP_CI][t % MOP_CI];
+    unsigned incl = mycnt;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const unsigned total = __shfl_sync(0xffffffffu, incl, 14);
+    if (total == 0) return;
+    __syncwarp();
+    if (lane < 15) pcnt[mypat] = incl - mycnt; // exclusive start of the bucket
+    __syncwarp();
+    const unsigned padded = (total + MOP_NG - 1) & ~(unsigned)(MOP_NG - 1);
+    nslots = (unsigned)__reduce_add_sync(0xffffffffu, nslots);
 
-    // ---- one unit per shift that occurred; its entries are copied out contiguously
-    while (shift_seen) {
-        unsigned sid = (unsigned)__ffs(shift_seen) - 1;
-        shift_seen &= shift_seen - 1;
-        unsigned cnt = 0;
-        for (int b = 0; b < nbuf; b += 32) {
-            int idx = b + lane;
-            bool m = idx < nbuf && binfo[idx] != 0xffffffffu && (binfo[idx] >> 16) == sid;
-            cnt += __popc(__ballot_sync(0xffffffffu, m));
-        }
-        if (cnt == 0) continue;
-        unsigned st = 0, ui = 0;
+    // ---- exclusion-mask rows of this i-octet, unit record, entries
+    unsigned mb = 0, st = 0, ui = 0;
+    if (lane == 0) {
+        atomicAdd(a.slots_active, (unsigned long long)nslots);
+        mb = atomicAdd(&a.ctr->n_masks, (unsigned)exN);
+        st = atomicAdd(&a.ctr->n_entries, padded);
+        ui = atomicAdd(&a.ctr->n_units, 1u);
+    }
+    mb = __shfl_sync(0xffffffffu, mb, 0);
+    st = __shfl_sync(0xffffffffu, st, 0);
+    ui = __shfl_sync(0xffffffffu, ui, 0);
+    const bool fits = mb + exN <= a.cap_masks && st + padded <= a.cap_entries && ui < a.cap_units;
+    if (!fits) {
         if (lane == 0) {
-            st = atomicAdd(&a.ctr->n_entries, cnt);
-            ui = atomicAdd(&a.ctr->n_units, 1u);
-        }
-        st = __shfl_sync(0xffffffffu, st, 0);
-        ui = __shfl_sync(0xffffffffu, ui, 0);
-        if (st + cnt > a.cap_entries || ui >= a.cap_units) {
-            if (lane == 0) atomicOr(&a.ctr->overflow, st + cnt > a.cap_entries ? 1u : 2u);
-            if (ui < a.cap_units && lane == 0) {
-                MopUnit un = {n, ci, (int)sid, 0u, 0u, mb, 0u, 0u};
+            atomicOr(&a.ctr->overflow, (mb + exN > a.cap_masks ? 4u : 0u) | (st + padded > a.cap_entries ? 1u : 0u) |
+                                           (ui >= a.cap_units ? 2u : 0u));
+            if (ui < a.cap_units) {
+                MopUnit un = {n, ci, 0u, 0u, 0u, 0u, 0u, 0u};
                 a.units[ui] = un;
             }
-            continue;
         }
-        unsigned wr = 0;
-        for (int b = 0; b < nbuf; b += 32) {
-            int idx = b + lane;
-            bool m = idx < nbuf && binfo[idx] != 0xffffffffu && (binfo[idx] >> 16) == sid;
-            unsigned bal = __ballot_sync(0xffffffffu, m);
-            if (m) {
-                unsigned pos = st + wr + __popc(bal & ((1u << lane) - 1));
-                a.entries[pos] = make_uint2((unsigned)bcj[idx], binfo[idx] & 0xffffu);
-            }
-            wr += __popc(bal);
-        }
-        if (lane == 0) {
-            MopUnit un = {n, ci, (int)sid, st, cnt, mb, 0u, 0u};
-            a.units[ui] = un;
-        }
+        return;
+    }
+    for (int t = lane; t < exN; t += 32)
+        a.masks[(size_t)mb + t] = (unsigned long long)exM[t][0] | ((unsigned long long)exM[t][1] << 32);
+    for (int idx = lane; idx < nbuf; idx += 32) {
+        const unsigned info = binfo[idx];
+        if (info == 0) continue;
+        const unsigned pos = st + pcnt[info & 15u] + (info >> 16);
+        a.entries[pos] = make_uint2(bcj[idx], info & 0xffffu);
+    }
+    if (lane < (int)(padded - total))
+        a.entries[st + total + lane] = make_uint2((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24), 0u);
+    if (lane == 0) {
+        MopUnit un = {n, ci, st, padded, mb, 0u, 0u, 0u};
+        a.units[ui] = un;
     }
 }
 
-__global__ void k_mark_bead0(MopCounters *ctr) { ctr->n_units_bead0 = min(ctr->n_units, 0xffffffffu); }
+__global__ void k_mark_bead0(MopCounters *ctr, unsigned cap_units) { ctr->n_units_bead0 = min(ctr->n_units, cap_units); }

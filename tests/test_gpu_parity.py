@@ -64,7 +64,7 @@ def test_cell_ids_and_stable_sort_bit_exact(B, oracle, name):
     m.mop_eval_veff_grad(R, want_grad=False)
     d = m.dims()
     dims = [d["nx"], d["ny"], d["nz"]]
-    assert dims == oracle.grid_dims(s.n_atoms, o.box, d["cj"], d["bin_z"])
+    assert dims == oracle.grid_dims(s.n_atoms, o.box, d["cluster"], d["bin_z"])
     cell = m.mop_debug_get("cell")
     perm = m.mop_debug_get("perm")
     xq = m.mop_debug_get("xq")
@@ -79,12 +79,12 @@ def test_cell_ids_and_stable_sort_bit_exact(B, oracle, name):
         # sorted coordinates are the wrapped ones, bit for bit; charges ride along
         assert np.array_equal(xq[n][real][:, :3], xw[p_ref])
         assert np.array_equal(xq[n][real][:, 3], np.asarray(s.charge, np.float32)[p_ref])
-        # padding only at column ends: inside a column the real slots come first, columns start at multiples of 32
+        # padding only at column ends: inside a column the real slots come first, columns start at multiples of 8
         col = c_ref[p_ref] // dims[2]
         slots = np.flatnonzero(real)
         for cc in np.unique(col)[:50]:
             sl = slots[col == cc]
-            assert sl[0] % 32 == 0 and np.array_equal(sl, np.arange(sl[0], sl[0] + len(sl)))
+            assert sl[0] % d["cluster"] == 0 and np.array_equal(sl, np.arange(sl[0], sl[0] + len(sl)))
     m.close()
 
 

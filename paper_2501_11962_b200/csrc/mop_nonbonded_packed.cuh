@@ -2,6 +2,7 @@
 // force-scalar + Hessian-vector pair kernel), SURVEY.md 8a.  FP32-pipe-bound; no tensor cores.
 #pragma once
 #include "mop_nonbonded.cuh"
+#include "mop_f2.cuh"
 
 // =====================================================================================================
 // Packed variant: two i atoms per lane per issue slot (sm_100a FFMA2 / FMUL2 / FADD2 = fma|mul|add.rn.f32x2).
@@ -15,39 +16,6 @@
 //   gn = -g = x (B - A) + C - 2 k_rf ke qi qj,      hn = -h = x (x (8A - 14B) - 3C),      dn = s_j - s_i = -delta
 //   F_i += gn d;                (H s)_i += hn (d.dn) d + gn dn;        the j side accumulates the same sums (jn),
 //   and the lane's j atom receives -(jn.lo + jn.hi) once per entry.
-typedef unsigned long long f2;
-__device__ __forceinline__ f2 f2_pack(float lo, float hi) {
-    f2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void f2_unpack(f2 v, float &lo, float &hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f2 f2_bc(float s) { return f2_pack(s, s); }
-__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
-    f2 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ void f2_acc(f2 &c, f2 a, f2 b) { // c += a * b, in place
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b));
-}
-__device__ __forceinline__ f2 f2_mul(f2 a, f2 b) {
-    f2 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
-    f2 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f2 f2_sub(f2 a, f2 b) {
-    f2 d;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
 // staging reads are volatile so that the compiler re-reads shared memory per entry instead of pinning the
 // eight i atoms in registers for the whole unit
 __device__ __forceinline__ float4 mop_lds_v4(unsigned addr) {

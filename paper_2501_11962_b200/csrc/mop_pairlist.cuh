@@ -12,6 +12,7 @@
 #pragma once
 #include "mop_common.cuh"
 #include "mop_nonbonded.cuh"
+#include "mop_f2.cuh"
 
 struct PlArgs {
     MopGrid g;
@@ -232,17 +233,18 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         nbuf = MOP_LBUF;
     }
 
-    // ---- phase 2: four candidates per step, lane = (j atom jl, candidate g): the 8 i atoms against the lane's j atom
-    // with the arithmetic of the pair kernels (xs_i = x_i - k L, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx)));
-    // pattern bit p = some pair of row pair p within r_list.  Padding atoms are never within range (mop_dummy_xq).
+    // ---- phase 2: four candidates per step, lane = (j atom jl, candidate g): the 8 i atoms (packed two by two, the
+    // row pairs of the pair kernels) against the lane's j atom with the arithmetic of the pair kernels
+    // (xs_i = x_i - k L, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx)); x - 0 = x exactly, so the steps without a
+    // shifted candidate skip the first subtraction); pattern bit p = some pair of row pair p within r_list.
+    // Padding atoms are never within range (mop_dummy_xq).
     const int gq = lane >> 3, jl = lane & 7;
-    float xi[MOP_CL], yi[MOP_CL], zi[MOP_CL];
+    f2 xi[4], yi[4], zi[4];
 #pragma unroll
-    for (int k = 0; k < MOP_CL; k++) {
-        const float4 p = xq[ci * MOP_CL + k];
-        xi[k] = p.x, yi[k] = p.y, zi[k] = p.z;
+    for (int p = 0; p < 4; p++) {
+        const float4 a0 = xq[ci * MOP_CL + 2 * p], a1 = xq[ci * MOP_CL + 2 * p + 1];
+        xi[p] = f2_pack(a0.x, a1.x), yi[p] = f2_pack(a0.y, a1.y), zi[p] = f2_pack(a0.z, a1.z);
     }
-    unsigned nslots = 0;
     for (int b = 0; b < nbuf; b += MOP_NG) {
         const int idx = b + gq;
         const bool live = idx < nbuf;
@@ -250,37 +252,55 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         const int cj = (int)(cw & 0xffffffu);
         const unsigned sid = cw >> 24;
         const float4 pj = xq[cj * MOP_CL + jl];
-        float sx, sy, sz;
-        mop_unit_shift((int)sid, g.box, sx, sy, sz);
+        const f2 jx = f2_bc(pj.x), jy = f2_bc(pj.y), jz = f2_bc(pj.z);
         unsigned pat = 0;
+        if (__any_sync(0xffffffffu, sid != MOP_NOSHIFT)) {
+            float sx, sy, sz;
+            mop_unit_shift((int)sid, g.box, sx, sy, sz);
+            const f2 hx = f2_bc(sx), hy = f2_bc(sy), hz = f2_bc(sz);
 #pragma unroll
-        for (int p = 0; p < 4; p++) {
-            bool in = false;
-#pragma unroll
-            for (int h = 0; h < 2; h++) {
-                const int k = 2 * p + h;
-                const float dx = __fsub_rn(__fsub_rn(xi[k], sx), pj.x), dy = __fsub_rn(__fsub_rn(yi[k], sy), pj.y),
-                            dz = __fsub_rn(__fsub_rn(zi[k], sz), pj.z);
-                in = in || (mop_r2(dx, dy, dz) < a.rl2);
+            for (int p = 0; p < 4; p++) {
+                const f2 dx = f2_sub(f2_sub(xi[p], hx), jx), dy = f2_sub(f2_sub(yi[p], hy), jy),
+                         dz = f2_sub(f2_sub(zi[p], hz), jz);
+                float r2a, r2b;
+                f2_unpack(f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx))), r2a, r2b);
+                const unsigned bal = __ballot_sync(0xffffffffu, fminf(r2a, r2b) < a.rl2);
+                if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
             }
-            const unsigned bal = __ballot_sync(0xffffffffu, in && live);
-            if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
+        } else {
+#pragma unroll
+            for (int p = 0; p < 4; p++) {
+                const f2 dx = f2_sub(xi[p], jx), dy = f2_sub(yi[p], jy), dz = f2_sub(zi[p], jz);
+                float r2a, r2b;
+                f2_unpack(f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx))), r2a, r2b);
+                const unsigned bal = __ballot_sync(0xffffffffu, fminf(r2a, r2b) < a.rl2);
+                if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
+            }
         }
-        // exclusion row of this octet pair (at most one row matches)
+        if (live && jl == 0) binfo[idx] = pat;
+    }
+    __syncwarp();
+
+    // ---- per candidate: exclusion row of its octet pair (at most one row matches) and position inside its pattern's
+    // bucket (lanes with equal patterns are ranked with one match; the first of them draws the range from the counter)
+    unsigned nslots = 0;
+    const unsigned pcnt_addr = (unsigned)__cvta_generic_to_shared(pcnt);
+    for (int b = 0; b < nbuf; b += 32) {
+        const int idx = b + lane;
+        unsigned pat = 0, cj = 0xffffffffu;
+        if (idx < nbuf) pat = binfo[idx], cj = bcj[idx] & 0xffffffu;
         unsigned row1 = 0;
-        for (int t0 = 0; t0 < exN; t0 += 8) {
-            const bool hit = pat != 0 && t0 + jl < exN && exJ[t0 + jl] == cj;
-            const unsigned hb = (__ballot_sync(0xffffffffu, hit) >> (8 * gq)) & 0xffu;
-            if (hb) row1 = (unsigned)(t0 + __ffs(hb));
-        }
-        if (live && jl == 0) {
-            unsigned info = 0;
-            if (pat != 0) {
-                const unsigned pos = atomicAdd(&pcnt[pat], 1u);
-                info = pat | (row1 << 8) | (pos << 16);
-                nslots += __popc(pat) * 16u;
-            }
-            binfo[idx] = info;
+        for (int t = 0; t < exN; t++)
+            if ((unsigned)exJ[t] == cj) row1 = (unsigned)t + 1u;
+        const unsigned same = __match_any_sync(0xffffffffu, pat);
+        const unsigned rank = __popc(same & ((1u << lane) - 1u));
+        unsigned base = 0;
+        if (rank == 0 && pat != 0)
+            asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(base) : "r"(pcnt_addr + pat * 4u), "r"(__popc(same)) : "memory");
+        base = __shfl_sync(0xffffffffu, base, __ffs(same) - 1);
+        if (pat != 0) {
+            binfo[idx] = pat | (row1 << 8) | ((base + rank) << 16);
+            nslots += __popc(pat) * 16u;
         }
     }
     __syncwarp();

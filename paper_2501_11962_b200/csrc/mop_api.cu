@@ -128,12 +128,14 @@ static cudaError_t dalloc(T **p, size_t n) {
 static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) / b); }
 
 typedef void (*nb_kernel_t)(const NbArgs);
-// the launched instances of the pair kernel (five resident CTAs per SM: 96 registers)
-#define NBP_CTAS 5
+// the launched instances of the pair kernel: six resident CTAs per SM (80 registers) for the force passes, five (96)
+// for the H.eta pass (measured: profiles/r02_experiments.md)
+#define NBP_CTAS_F 6
+#define NBP_CTAS_H 5
 static nb_kernel_t nb_pick(int mode, bool count = false) {
-    if (count) return k_nonbonded_p<NB_FORCE, true, NBP_CTAS>;
-    return mode == NB_FORCE ? k_nonbonded_p<NB_FORCE, false, NBP_CTAS>
-         : mode == NB_ENERGY ? k_nonbonded_p<NB_ENERGY, false, NBP_CTAS> : k_nonbonded_p<NB_HVP, false, NBP_CTAS>;
+    if (count) return k_nonbonded_p<NB_FORCE, true, NBP_CTAS_F>;
+    return mode == NB_FORCE ? k_nonbonded_p<NB_FORCE, false, NBP_CTAS_F>
+         : mode == NB_ENERGY ? k_nonbonded_p<NB_ENERGY, false, NBP_CTAS_F> : k_nonbonded_p<NB_HVP, false, NBP_CTAS_H>;
 }
 static size_t nb_smem(const mop_ctx *c) { return nbp_smem_bytes(c->nt); }
 
@@ -494,13 +496,13 @@ static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.slots_active = c->d_slots;
     a.cap_units = c->cap_units, a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks;
-    const unsigned nci_blocks = cdiv(g.S / MOP_CL, 4);
+    const unsigned nci_blocks = cdiv(g.S / MOP_CL, MOP_PL_WARPS);
     a.bead0 = 0;
-    LAUNCH(c, k_pairlist, dim3(nci_blocks, 1), 128, 0, a); // bead 1 first: its units come first (energy variant)
+    LAUNCH(c, k_pairlist, dim3(nci_blocks, 1), 32 * MOP_PL_WARPS, 0, a); // bead 1 first: its units come first (energy variant)
     LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr, c->cap_units);
     if (nb > 1) {
         a.bead0 = 1;
-        LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 128, 0, a);
+        LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 32 * MOP_PL_WARPS, 0, a);
     }
     c->n_rebuilds += 1;
     if (timed) t_mark(c, 2);

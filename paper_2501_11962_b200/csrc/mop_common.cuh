@@ -18,8 +18,8 @@
 #define MOP_KE 138.935458f // Coulomb constant, kJ mol^-1 nm e^-2
 #define MOP_MAX_TYPES 64
 #define MOP_EXROWS 48      // max distinct j-octets holding exclusion partners of one i-octet (row 0: the octet itself)
-#define MOP_LBUF 512       // per-warp staging capacity (candidate j-octets) in the list builder
-#define MOP_NOSHIFT 13     // shift id (kx+1) + 3 (ky+1) + 9 (kz+1) of the zero shift
+#define MOP_LBUF 384       // per-warp staging capacity (candidate j-octets) in the list builder
+#define MOP_NOSHIFT 21     // shift id (kx+1) | (ky+1) << 2 | (kz+1) << 4 of the zero shift
 
 struct MopGrid {
     float box[3], inv_box[3]; // inv_box = 1.0f / box (FP32)
@@ -39,9 +39,11 @@ struct MopUnit {            // one work unit of the pair kernels: (bead, i-octet
     unsigned pad0, pad1, pad2;
 };
 
-// entry: x = j-octet index within the bead | shift id << 24  ((kx+1) + 3 (ky+1) + 9 (kz+1), MOP_NOSHIFT = none)
+// entry: x = j-octet index within the bead | shift id << 24  ((kx+1) | (ky+1) << 2 | (kz+1) << 4, MOP_NOSHIFT = none)
 //        y = pattern (bits 0-3: row pair p = i atoms (2p, 2p+1) has a pair within r_list of this octet; 0: padding)
-//            | (exclusion row + 1) << 8 (0: no exclusions in this octet pair)
+//            | (exclusion row + 1) << 8 (bits 8-15; 0: no exclusions in this octet pair)
+//            | step information, the same in the four entries of a step: bits 16-19 union of their patterns,
+//              bit 20 some entry is shifted, bit 21 some entry has an exclusion row or is padding
 // The entries of a unit are ordered by pattern, so that the four octets of a warp step mostly share theirs.
 typedef uint2 MopEntry;
 

@@ -22,7 +22,7 @@ struct NbArgs {
     float4 *out;        // [nf][S] F4 or H4, accumulated with vector reductions
     const MopUnit *units;
     const MopEntry *entries;
-    const unsigned long long *masks; // exclusion rows: byte k = the j slots (bits 0-7) i atom k may interact with
+    const unsigned long long *masks; // exclusion rows: byte jl = the i atoms (bits 0-7) j atom jl may interact with
     const MopCounters *ctr;
     unsigned cap_units;              // units beyond the allocation were never written (overflow): never read them
     unsigned long long *n_inrange;   // counting variant only: in-range, non-excluded pair decisions of this launch
@@ -47,9 +47,9 @@ __device__ __forceinline__ float mop_r2(float dx, float dy, float dz) {
 }
 
 __device__ __forceinline__ void mop_unit_shift(int s, const float box[3], float &sx, float &sy, float &sz) {
-    sx = (float)(s % 3 - 1) * box[0];
-    sy = (float)((s / 3) % 3 - 1) * box[1];
-    sz = (float)(s / 9 - 1) * box[2];
+    sx = (float)((s & 3) - 1) * box[0];
+    sy = (float)(((s >> 2) & 3) - 1) * box[1];
+    sz = (float)((s >> 4) - 1) * box[2];
 }
 
 // ---- debug: the set of in-range, non-excluded pairs of one bead, scalar restatement of the predicate over the list ----
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(128) k_debug_pairs(const PairDbgArgs a) {
             const MopEntry cur = a.entries[e0 + g];
             const unsigned pat = cur.y & 15u;
             if (pat == 0) continue;
-            const unsigned oc = cur.x & 0xffffffu, sid = cur.x >> 24, row1 = cur.y >> 8;
+            const unsigned oc = cur.x & 0xffffffu, sid = cur.x >> 24, row1 = (cur.y >> 8) & 0xffu;
             float sx, sy, sz;
             mop_unit_shift((int)sid, a.box, sx, sy, sz);
             const float4 cp = xq[(size_t)oc * MOP_CL + jl];
@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(128) k_debug_pairs(const PairDbgArgs a) {
             for (int k = 0; k < MOP_CL; k++) {
                 if (!((pat >> (k >> 1)) & 1u)) continue;
                 const float4 pi = xq[un.ci * MOP_CL + k];
-                const bool allowed = (row >> (8 * k + jl)) & 1ull;
+                const bool allowed = (row >> (8 * jl + k)) & 1ull;
                 const float dx = __fsub_rn(__fsub_rn(pi.x, sx), cp.x), dy = __fsub_rn(__fsub_rn(pi.y, sy), cp.y),
                             dz = __fsub_rn(__fsub_rn(pi.z, sz), cp.z);
                 const float r2 = mop_r2(dx, dy, dz);

@@ -44,19 +44,6 @@ __device__ __forceinline__ uint2 mop_lds_vu2(unsigned addr) {
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
     return v;
 }
-// asynchronous global -> shared copies (LDGSTS): the j atoms of the entries ahead are in flight while one is processed
-__device__ __forceinline__ void mop_cp_async16(unsigned saddr, const void *g) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(g) : "memory");
-}
-__device__ __forceinline__ void mop_cp_async4(unsigned saddr, const void *g) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(saddr), "l"(g) : "memory");
-}
-__device__ __forceinline__ void mop_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void mop_cp_wait() {
-    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-}
-
 #define NBP_NST 2       // stages of the per-warp j-atom ring (steps in flight: NBP_NST - 1)
 
 // Shared memory of one CTA (4 warps), bytes:
@@ -122,8 +109,8 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     // one step: the lane's j atom (cp, ce, type offset tj4) against the row pairs of the union pattern `upat`.
     // sh*: the lane's periodic shift (packed broadcast; zero for most steps: x - 0 = x exactly, so one code path
     // serves both, the shifted form only being compiled into the SHIFTED instance).
-    auto step = [&](const uint2 cur, const unsigned upat, const bool shifted, const float4 cp, const float4 ce,
-                    const unsigned tj4) {
+    auto step = [&](const uint2 cur, const unsigned upat, const bool shifted, const bool masked, const float4 cp,
+                    const float4 ce, const unsigned tj4) {
         const f2 jx = f2_bc(cp.x), jy = f2_bc(cp.y), jz = f2_bc(cp.z), jq = f2_bc(cp.w);
         f2 shx = 0ull, shy = 0ull, shz = 0ull;
         if (shifted) {
@@ -137,12 +124,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         // (a padding entry -- pattern 0, it points at the unit's own octet -- allows nothing)
         const bool valid = (cur.y & 15u) != 0u;
         unsigned lm = valid ? 0xffu : 0u;
-        const unsigned row1 = cur.y >> 8;
-        const bool masked = __any_sync(0xffffffffu, row1 != 0 || !valid);
-        if (masked && row1 != 0) {
-            const unsigned long long row = a.masks[(size_t)un.excl_base + row1 - 1];
-            const unsigned w0 = ((unsigned)row >> jl) & 0x01010101u, w1 = ((unsigned)(row >> 32) >> jl) & 0x01010101u;
-            lm = ((w0 | (w0 >> 7) | (w0 >> 14) | (w0 >> 21)) & 0xfu) | (((w1 | (w1 >> 7) | (w1 >> 14) | (w1 >> 21)) & 0xfu) << 4);
+        if (masked) {
+            const unsigned row1 = (cur.y >> 8) & 0xffu;
+            if (row1 != 0)
+                lm = reinterpret_cast<const unsigned char *>(a.masks)[((size_t)un.excl_base + row1 - 1) * 8 + jl];
         }
 
         auto heavy = [&](const int p, const bool nolj) {
@@ -282,10 +267,12 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             } else {
                 tj4 = mop_lds_vu(st + 512u + lane * 4) * 4u;
             }
-            const unsigned upat = __reduce_or_sync(0xffffffffu, cur.y & 15u);
-            const bool shifted = __any_sync(0xffffffffu, (cur.x >> 24) != MOP_NOSHIFT);
-            if (shifted) step(cur, upat, true, cp, ce, tj4);
-            else step(cur, upat, false, cp, ce, tj4);
+            // step information from the list builder, the same in all four entries (warp-uniform by construction)
+            const unsigned upat = (cur.y >> 16) & 15u;
+            const bool shifted = (cur.y >> 20) & 1u, masked = (cur.y >> 21) & 1u;
+            if (shifted) step(cur, upat, true, true, cp, ce, tj4);
+            else if (masked) step(cur, upat, false, true, cp, ce, tj4);
+            else step(cur, upat, false, false, cp, ce, tj4);
         }
         mop_cp_wait<0>();
     }

@@ -39,18 +39,20 @@ __device__ __forceinline__ float mop_gap(float lo_a, float hi_a, float lo_b, flo
 // row pairs of an octet being ordered along z), then the rest
 __constant__ unsigned char c_pat_order[16] = {15, 7, 3, 1, 14, 12, 8, 6, 2, 4, 5, 9, 10, 11, 13, 0};
 
-__global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
-    __shared__ int s_exJ[4][MOP_EXROWS];
-    __shared__ unsigned s_exM[4][MOP_EXROWS][2];
-    __shared__ int s_exN[4];
-    __shared__ unsigned s_bcj[4][MOP_LBUF];
-    __shared__ unsigned s_binfo[4][MOP_LBUF];
-    __shared__ unsigned s_pcnt[4][16];
+#define MOP_PL_WARPS 4     // warps (i-octets) per CTA of the list builder
+__global__ void __launch_bounds__(32 * MOP_PL_WARPS) k_pairlist(PlArgs a) {
+    __shared__ int s_exJ[MOP_PL_WARPS][MOP_EXROWS];
+    __shared__ unsigned s_exM[MOP_PL_WARPS][MOP_EXROWS][2];
+    __shared__ int s_exN[MOP_PL_WARPS];
+    __shared__ unsigned s_bcj[MOP_PL_WARPS][MOP_LBUF];
+    __shared__ unsigned s_binfo[MOP_PL_WARPS][MOP_LBUF];
+    __shared__ unsigned s_pcnt[MOP_PL_WARPS][32];
+    __shared__ float4 s_j[MOP_PL_WARPS][32 * 9];
 
     const MopGrid &g = a.g;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n = a.bead0 + blockIdx.y;
-    const int ci = blockIdx.x * 4 + w;
+    const int ci = blockIdx.x * MOP_PL_WARPS + w;
     const int noc = g.S / MOP_CL;
     if (ci >= noc) return;
     const float4 blo = a.blo[(size_t)n * noc + ci], bhi = a.bhi[(size_t)n * noc + ci];
@@ -64,6 +66,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
     int *exJ = s_exJ[w];
     unsigned(*exM)[2] = s_exM[w];
     unsigned *bcj = s_bcj[w], *binfo = s_binfo[w], *pcnt = s_pcnt[w];
+    float4 *sj = s_j[w];
     const int J0 = ci;
 
     if (lane < MOP_EXROWS) {
@@ -80,7 +83,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         exM[lane][1] = lane == 0 ? hi : 0xffffffffu;
     }
     for (int t = 32 + lane; t < MOP_EXROWS; t += 32) exM[t][0] = exM[t][1] = 0xffffffffu;
-    if (lane < 16) pcnt[lane] = 0;
+    pcnt[lane] = 0;
     if (lane == 0) {
         exJ[0] = J0;
         s_exN[w] = 1;
@@ -180,7 +183,7 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
                         if (r1 > r0) {
                             first = max((s0 + r0) >> 3, J0); // half list: never below the own octet
                             cnt = max(((s0 + r1 - 1) >> 3) - first + 1, 0);
-                            sid = (unsigned)((kx + 1) + 3 * (ky + 1) + 9 * (kz + 1));
+                            sid = (unsigned)((kx + 1) | ((ky + 1) << 2) | ((kz + 1) << 4));
                         }
                     }
                 }
@@ -228,16 +231,17 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         }
     }
     __syncwarp();
-    if (nbuf > MOP_LBUF) {
+    if (nbuf > MOP_LBUF) { // candidates beyond the staging capacity were dropped
         if (lane == 0) atomicOr(&a.ctr->overflow, 8u);
-        nbuf = MOP_LBUF;
+        return;
     }
 
-    // ---- phase 2: four candidates per step, lane = (j atom jl, candidate g): the 8 i atoms (packed two by two, the
-    // row pairs of the pair kernels) against the lane's j atom with the arithmetic of the pair kernels
-    // (xs_i = x_i - k L, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx)); x - 0 = x exactly, so the steps without a
-    // shifted candidate skip the first subtraction); pattern bit p = some pair of row pair p within r_list.
-    // Padding atoms are never within range (mop_dummy_xq).
+    // ---- phase 2: one candidate per lane.  The 8 i atoms (packed two by two: the row pairs of the pair kernels)
+    // against the 8 atoms of the lane's j-octet, with the arithmetic of the pair kernels (xs_i = x_i - k L -- x - 0 = x
+    // exactly for the zero shift --, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx))); pattern bit p = some pair of
+    // row pair p within r_list.  Padding atoms are never within range (mop_dummy_xq).  Then the exclusion row of the
+    // octet pair (at most one matches) and the position inside the bucket of (pattern, shifted or not): lanes with
+    // equal keys are ranked with one match, the first of them draws the range from the bucket's counter.
     const int gq = lane >> 3, jl = lane & 7;
     f2 xi[4], yi[4], zi[4];
 #pragma unroll
@@ -245,82 +249,77 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         const float4 a0 = xq[ci * MOP_CL + 2 * p], a1 = xq[ci * MOP_CL + 2 * p + 1];
         xi[p] = f2_pack(a0.x, a1.x), yi[p] = f2_pack(a0.y, a1.y), zi[p] = f2_pack(a0.z, a1.z);
     }
-    for (int b = 0; b < nbuf; b += MOP_NG) {
-        const int idx = b + gq;
-        const bool live = idx < nbuf;
-        const unsigned cw = live ? bcj[idx] : ((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24));
-        const int cj = (int)(cw & 0xffffffu);
-        const unsigned sid = cw >> 24;
-        const float4 pj = xq[cj * MOP_CL + jl];
-        const f2 jx = f2_bc(pj.x), jy = f2_bc(pj.y), jz = f2_bc(pj.z);
-        unsigned pat = 0;
-        if (__any_sync(0xffffffffu, sid != MOP_NOSHIFT)) {
-            float sx, sy, sz;
-            mop_unit_shift((int)sid, g.box, sx, sy, sz);
-            const f2 hx = f2_bc(sx), hy = f2_bc(sy), hz = f2_bc(sz);
-#pragma unroll
-            for (int p = 0; p < 4; p++) {
-                const f2 dx = f2_sub(f2_sub(xi[p], hx), jx), dy = f2_sub(f2_sub(yi[p], hy), jy),
-                         dz = f2_sub(f2_sub(zi[p], hz), jz);
-                float r2a, r2b;
-                f2_unpack(f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx))), r2a, r2b);
-                const unsigned bal = __ballot_sync(0xffffffffu, fminf(r2a, r2b) < a.rl2);
-                if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
-            }
-        } else {
-#pragma unroll
-            for (int p = 0; p < 4; p++) {
-                const f2 dx = f2_sub(xi[p], jx), dy = f2_sub(yi[p], jy), dz = f2_sub(zi[p], jz);
-                float r2a, r2b;
-                f2_unpack(f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx))), r2a, r2b);
-                const unsigned bal = __ballot_sync(0xffffffffu, fminf(r2a, r2b) < a.rl2);
-                if ((bal >> (8 * gq)) & 0xffu) pat |= 1u << p;
-            }
-        }
-        if (live && jl == 0) binfo[idx] = pat;
-    }
-    __syncwarp();
-
-    // ---- per candidate: exclusion row of its octet pair (at most one row matches) and position inside its pattern's
-    // bucket (lanes with equal patterns are ranked with one match; the first of them draws the range from the counter)
     unsigned nslots = 0;
     const unsigned pcnt_addr = (unsigned)__cvta_generic_to_shared(pcnt);
     for (int b = 0; b < nbuf; b += 32) {
         const int idx = b + lane;
-        unsigned pat = 0, cj = 0xffffffffu;
-        if (idx < nbuf) pat = binfo[idx], cj = bcj[idx] & 0xffffffu;
+        const bool live = idx < nbuf;
+        const unsigned cw = live ? bcj[idx] : ((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24));
+        const unsigned cj = cw & 0xffffffu, sid = cw >> 24;
+        float sx, sy, sz;
+        mop_unit_shift((int)sid, g.box, sx, sy, sz);
+        const f2 hx = f2_bc(sx), hy = f2_bc(sy), hz = f2_bc(sz);
+        f2 xs[4], ys[4], zs[4];
+#pragma unroll
+        for (int p = 0; p < 4; p++) xs[p] = f2_sub(xi[p], hx), ys[p] = f2_sub(yi[p], hy), zs[p] = f2_sub(zi[p], hz);
+        float best[4] = {3.0e38f, 3.0e38f, 3.0e38f, 3.0e38f}; // smallest r2 of each row pair
+        // the 32 candidates' octets go through shared memory: coalesced loads (lane = (atom jl, candidate 4 t + gq)),
+        // then every lane reads the 8 atoms of its own candidate (row stride 9 float4: conflict-free)
+        __syncwarp();
+#pragma unroll
+        for (int t = 0; t < 8; t++) {
+            const unsigned cwt = __shfl_sync(0xffffffffu, cw, 4 * t + gq);
+            sj[(4 * t + gq) * 9 + jl] = xq[(size_t)(cwt & 0xffffffu) * MOP_CL + jl];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < MOP_CL; j++) {
+            const float4 q = sj[lane * 9 + j];
+            const f2 jx = f2_bc(q.x), jy = f2_bc(q.y), jz = f2_bc(q.z);
+#pragma unroll
+            for (int p = 0; p < 4; p++) {
+                const f2 dx = f2_sub(xs[p], jx), dy = f2_sub(ys[p], jy), dz = f2_sub(zs[p], jz);
+                float r2a, r2b;
+                f2_unpack(f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx))), r2a, r2b);
+                best[p] = fminf(best[p], fminf(r2a, r2b));
+            }
+        }
+        unsigned pat = 0;
+#pragma unroll
+        for (int p = 0; p < 4; p++)
+            if (best[p] < a.rl2) pat |= 1u << p;
+        if (!live) pat = 0;
         unsigned row1 = 0;
         for (int t = 0; t < exN; t++)
             if ((unsigned)exJ[t] == cj) row1 = (unsigned)t + 1u;
-        const unsigned same = __match_any_sync(0xffffffffu, pat);
+        const unsigned key = pat == 0 ? 0u : (pat | (sid != MOP_NOSHIFT ? 16u : 0u));
+        const unsigned same = __match_any_sync(0xffffffffu, key);
         const unsigned rank = __popc(same & ((1u << lane) - 1u));
         unsigned base = 0;
-        if (rank == 0 && pat != 0)
-            asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(base) : "r"(pcnt_addr + pat * 4u), "r"(__popc(same)) : "memory");
+        if (rank == 0 && key != 0)
+            asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(base) : "r"(pcnt_addr + key * 4u), "r"(__popc(same)) : "memory");
         base = __shfl_sync(0xffffffffu, base, __ffs(same) - 1);
-        if (pat != 0) {
-            binfo[idx] = pat | (row1 << 8) | ((base + rank) << 16);
-            nslots += __popc(pat) * 16u;
-        }
+        if (live) binfo[idx] = key == 0 ? 0u : (key | (row1 << 8) | ((base + rank) << 16));
+        nslots += __popc(pat) * 16u;
     }
     __syncwarp();
 
-    // ---- bucket starts in pattern order, total, padded total
-    unsigned mycnt = 0, mypat = 0;
-    if (lane < 15) {
-        mypat = c_pat_order[lane];
-        mycnt = pcnt[mypat];
+    // ---- bucket starts in (pattern order, plain before shifted), total, padded total
+    unsigned mycnt = 0, mykey = 0;
+    if (lane < 30) {
+        mykey = (unsigned)c_pat_order[lane >> 1] | ((lane & 1) << 4);
+        mycnt = pcnt[mykey];
     }
     unsigned incl = mycnt;
 #pragma unroll
-    for (int o = 1; o < 16; o <<= 1) {
+    for (int o = 1; o < 32; o <<= 1) {
         const unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
         if (lane >= o) incl += v;
     }
-    const unsigned total = __shfl_sync(0xffffffffu, incl, 14);
+    const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
     if (total == 0) return;
     __syncwarp();
-    if (lane < 15) pcnt[mypat] = incl - mycnt; // exclusive start of the bucket
+    if (lane < 30) pcnt[mykey] = incl - mycnt; // exclusive start of the bucket
     __syncwarp();
     const unsigned padded = (total + MOP_NG - 1) & ~(unsigned)(MOP_NG - 1);
     nslots = (unsigned)__reduce_add_sync(0xffffffffu, nslots);
@@ -348,16 +347,42 @@ __global__ void __launch_bounds__(128) k_pairlist(PlArgs a) {
         }
         return;
     }
-    for (int t = lane; t < exN; t += 32)
-        a.masks[(size_t)mb + t] = (unsigned long long)exM[t][0] | ((unsigned long long)exM[t][1] << 32);
+    // mask rows leave transposed: byte jl of the 64-bit row = the i atoms (bits 0-7) j atom jl may interact with, so
+    // that a lane of the pair kernels reads its 8 bits with one byte load (8x8 bit-matrix transpose, three swaps)
+    for (int t = lane; t < exN; t += 32) {
+        unsigned long long x = (unsigned long long)exM[t][0] | ((unsigned long long)exM[t][1] << 32), y;
+        y = (x ^ (x >> 7)) & 0x00AA00AA00AA00AAull, x ^= y ^ (y << 7);
+        y = (x ^ (x >> 14)) & 0x0000CCCC0000CCCCull, x ^= y ^ (y << 14);
+        y = (x ^ (x >> 28)) & 0x00000000F0F0F0F0ull, x ^= y ^ (y << 28);
+        a.masks[(size_t)mb + t] = x;
+    }
+    // entries in their final order go through shared memory (the j staging buffer is free now), so that every step of
+    // four can be given its union pattern and flags: y bits 16-19 union of the four patterns, bit 20 some entry of the
+    // step is shifted, bit 21 some entry has an exclusion row or is padding.  The pair kernels branch on these.
+    __syncwarp();
+    uint2 *sorted = reinterpret_cast<uint2 *>(sj);
     for (int idx = lane; idx < nbuf; idx += 32) {
         const unsigned info = binfo[idx];
         if (info == 0) continue;
-        const unsigned pos = st + pcnt[info & 15u] + (info >> 16);
-        a.entries[pos] = make_uint2(bcj[idx], info & 0xffffu);
+        sorted[pcnt[info & 31u] + (info >> 16)] = make_uint2(bcj[idx], info & 0xff0fu);
     }
-    if (lane < (int)(padded - total))
-        a.entries[st + total + lane] = make_uint2((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24), 0u);
+    if (lane < (int)(padded - total)) sorted[total + lane] = make_uint2((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24), 0u);
+    __syncwarp();
+    for (unsigned sidx = lane; sidx < padded / MOP_NG; sidx += 32) {
+        uint2 e[MOP_NG];
+        unsigned u = 0, fl = 0;
+#pragma unroll
+        for (int q = 0; q < MOP_NG; q++) {
+            e[q] = sorted[sidx * MOP_NG + q];
+            u |= e[q].y & 15u;
+            if ((e[q].x >> 24) != MOP_NOSHIFT) fl |= 1u << 20;
+            if ((e[q].y >> 8) != 0u || (e[q].y & 15u) == 0u) fl |= 1u << 21;
+        }
+        fl |= u << 16;
+        uint4 *dst = reinterpret_cast<uint4 *>(a.entries + st + sidx * MOP_NG); // st is a multiple of 4: 32 B aligned
+        dst[0] = make_uint4(e[0].x, e[0].y | fl, e[1].x, e[1].y | fl);
+        dst[1] = make_uint4(e[2].x, e[2].y | fl, e[3].x, e[3].y | fl);
+    }
     if (lane == 0) {
         MopUnit un = {n, ci, st, padded, mb, 0u, 0u, 0u};
         a.units[ui] = un;

@@ -330,6 +330,89 @@ def test_P11_zero_length_harmonic_dimer(oracle):
     assert np.allclose(G3, 3.0 * G, rtol=1e-10, atol=1e-9)
 
 
+def _rotation(seed):
+    """A proper rotation matrix from a seeded QR (so that no closed-form pin is axis-aligned by accident)."""
+    q, r = np.linalg.qr(np.random.default_rng(seed).normal(size=(3, 3)))
+    q = q * np.sign(np.diag(r))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    return q
+
+
+@pytest.mark.parametrize("rot", [None, 1, 2])
+def test_P16_harmonic_bond_closed_form(oracle, rot):
+    """Two bonded atoms, b0 = 0.125 nm, k_b = 1e5, r = 0.140625 nm (all exact in FP32; values from
+    tests/golden/make_golden.py, formulas only): U = k_b/2 (r-b0)^2 = 12.207, |F| = k_b (r-b0) = 1562.5 along the bond
+    and attractive, curvature k_b along the bond and
+    k_b (1 - b0/r) across it.  Fixes b0, k_b, their order in the parameter pair, and the sign of the force."""
+    Q = np.eye(3) if rot is None else _rotation(rot)
+    u = Q @ np.array([1.0, 0.0, 0.0])
+    t = Q @ np.array([0.0, 1.0, 0.0])
+    X = np.array([[2.0, 2.0, 2.0], [2.0, 2.0, 2.0] + 0.140625 * u])
+    s = H.make_system("bond", [5.0] * 3, X, [12.0, 3.0], [0, 0], [0, 0], [0.3], [0.0], bonds=[[0, 1]],
+                      bpar=[[0.125, 1.0e5]], r_cut=1.0)
+    o = oracle.OracleSystem(s)
+    sv = np.zeros((2, 3))
+    sv[0] = u
+    res = oracle.bead(o, X, geom=0, brute=True, s=sv)
+    assert res["U"][2] == pytest.approx(GOLD["bond_U"], rel=1e-12) and res["U"][0] == 0 and res["U"][1] == 0
+    assert np.allclose(res["F"][0], GOLD["bond_F"] * u, rtol=1e-10, atol=1e-9)      # atom 0 is pulled towards atom 1
+    assert np.allclose(res["F"][1], -GOLD["bond_F"] * u, rtol=1e-10, atol=1e-9)
+    assert np.allclose(res["Hs"][0], GOLD["bond_kpar"] * u, rtol=1e-10, atol=1e-6)  # displacement along the bond
+    assert np.allclose(res["Hs"][1], -GOLD["bond_kpar"] * u, rtol=1e-10, atol=1e-6)
+    sv[0] = t
+    res = oracle.bead(o, X, geom=0, brute=True, s=sv)
+    assert np.allclose(res["Hs"][0], GOLD["bond_kperp"] * t, rtol=1e-10, atol=1e-6)  # displacement across the bond
+    # compressed bond: repulsive, same magnitude law
+    X2 = np.array([[2.0, 2.0, 2.0], [2.0, 2.0, 2.0] + 0.109375 * u])
+    res = oracle.bead(o, X2, geom=0, brute=True)
+    assert np.allclose(res["F"][0], -1.0e5 * 0.015625 * u, rtol=1e-9, atol=1e-8)
+    assert res["U"][2] == pytest.approx(0.5 * 1.0e5 * 0.015625 ** 2, rel=1e-10)
+
+
+@pytest.mark.parametrize("deg", [90, 150])
+@pytest.mark.parametrize("rot", [None, 3])
+def test_P16_harmonic_angle_closed_form(oracle, deg, rot):
+    """Three atoms i-j-k, j central, |a| = 0.1, |b| = 0.15, theta0 = 1.875 rad (107.43 deg, exact in FP32), k_theta = 383, at
+    theta = 90 deg (opens) and 150 deg (closes): U = k/2 (theta-theta0)^2, F_i perpendicular to a in the plane with
+    |F_i| = k |theta-theta0| / |a|, F_k likewise with |b|, F_j = -F_i - F_k (tests/golden/make_golden.py, formulas
+    only).  Fixes theta0, k_theta, which atom is central, the angle convention (not its supplement) and the signs."""
+    Q = np.eye(3) if rot is None else _rotation(rot)
+    th = np.deg2rad(deg)
+    rj = np.array([2.0, 2.2, 1.9])
+    ri = rj + Q @ (0.1 * np.array([1.0, 0.0, 0.0]))
+    rk = rj + Q @ (0.15 * np.array([np.cos(th), np.sin(th), 0.0]))
+    gold = {n: Q @ np.array([GOLD["angle%d_%s%s" % (deg, n, ax)] for ax in "xyz"]) for n in ("Fi", "Fj", "Fk")}
+    for order in ((0, 1, 2), (2, 1, 0)):        # (i, j, k) and the same angle named (k, j, i): identical physics
+        X = np.zeros((3, 3))
+        X[order[0]], X[order[1]], X[order[2]] = ri, rj, rk
+        s = H.make_system("angle", [5.0] * 3, X, [12.0, 3.0, 5.0], [0, 0, 0], [0, 0, 0], [0.3], [0.0],
+                          angles=[[order[0], order[1], order[2]]], apar=[[1.875, 383.0]], r_cut=1.0,
+                          excl=W.exclusions_from_bonds(3, [[0, 1], [1, 2]]))
+        o = oracle.OracleSystem(s)
+        res = oracle.bead(o, X, geom=0, brute=True)
+        assert res["U"][3] == pytest.approx(GOLD["angle%d_U" % deg], rel=1e-12)
+        assert res["U"][0] == 0 and res["U"][1] == 0 and res["U"][2] == 0
+        for n, idx in (("Fi", order[0]), ("Fj", order[1]), ("Fk", order[2])):
+            assert np.allclose(res["F"][idx], gold[n], rtol=1e-10, atol=1e-8), (n, res["F"][idx], gold[n])
+    # the force on i does no work along a (pure rotation) and opens (90 deg) or closes (150 deg) the angle
+    assert abs(gold["Fi"] @ (ri - rj)) < 1e-9
+    assert np.sign(gold["Fi"] @ (rk - rj)) == (1.0 if deg == 150 else -1.0)
+
+
+def test_G13_grid_dimensions_and_cell_ids_by_hand(oracle):
+    """Search-grid dimensions and cell ids on a hand-sized case: box 3 x 4 x 5, Q = 1000, cluster 8, z bins 0.125:
+    side = cbrt(8 * 60 / 1000) = 0.78297..., nx = floor(3 / side) = 3, ny = floor(4 / side) = 5, nz = floor(5 / 0.125) = 40;
+    cell = (cx ny + cy) nz + cz with c = floor(x n / L)."""
+    box = np.array([3.0, 4.0, 5.0], np.float32)
+    assert oracle.grid_dims(1000, box, 8, 0.125) == [3, 5, 40]
+    assert oracle.grid_dims(125, box, 8, 0.125)[:2] == [1, 2]          # side = cbrt(3.84) = 1.566: floor(3/1.566), floor(4/1.566)
+    X = np.array([[0.1, 0.1, 0.1], [2.9, 3.9, 4.9], [1.5, 2.0, 2.5], [2.1, 0.7, 0.2]], np.float32)
+    cell = oracle.cell_ids(X, box, [3, 5, 40])
+    #            (0,0,0)   (2,4,39)               (1,2,20)               (2,0,1)
+    assert cell.tolist() == [0, (2 * 5 + 4) * 40 + 39, (1 * 5 + 2) * 40 + 20, (2 * 5 + 0) * 40 + 1]
+
+
 # ---------------------------------------------------------------- P12 integrator
 def test_P12_velocity_verlet_invariants(oracle):
     s = H.lj_cluster(32)

@@ -142,16 +142,19 @@ void orc_stable_sort_by_cell(const int *cell, int Q, int ncell, int *perm) {
 }
 
 /* FP32 pair predicate for a given image shift k (each in {-1,0,1}), reading G8:
- *   xs_i = xw_i - k*L         (k*L exact, one rounding)
- *   d    = xs_i - xw_j        (one rounding)
- *   r2 = fma(dz,dz, fma(dy,dy, dx*dx));   in range iff r2 < rc*rc          */
+ *   d0 = xw_i - xw_j          (one rounding)
+ *   d  = d0 - k*L             (k*L exact, one rounding; k = 0: d = d0 exactly)
+ *   r2 = fma(dz,dz, fma(dy,dy, dx*dx));   in range iff r2 < rc*rc
+ * Both roundings are odd functions of their operands, so swapping the two atoms (k -> -k) gives -d
+ * bit for bit and the same r2: membership is a property of the unordered pair, whichever atom an
+ * implementation chooses to call i.                                                              */
 static int orc_pred_f32(const float *xi, const float *xj, const float box[3], const int k[3],
                         float rc2, float *r2out) {
     float d[3];
     for (int a = 0; a < 3; a++) {
         float s = (float)k[a] * box[a];
-        float xs = xi[a] - s;
-        d[a] = xs - xj[a];
+        float d0 = xi[a] - xj[a];
+        d[a] = d0 - s;
     }
     float r2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
     if (r2out) *r2out = r2;

@@ -40,8 +40,9 @@ __device__ __forceinline__ float mop_rsqrt(float x) {
     return y;
 }
 
-// G8: the pair predicate.  xs_i = xw_i - k L (k L exact, one rounding; xs_i = xw_i exactly for the zero shift); then
-// d = xs_i - xw_j (one rounding per component), r2 = fma(dz,dz, fma(dy,dy, dx*dx)), in range iff r2 < rc*rc.
+// G8: the pair predicate.  d = (xw_i - xw_j) - k L (one rounding each; k L exact; d = xw_i - xw_j exactly for the zero
+// shift), r2 = fma(dz,dz, fma(dy,dy, dx*dx)), in range iff r2 < rc*rc.  Swapping the roles of the two atoms (k -> -k)
+// negates d bit for bit, so the result does not depend on which atom of a pair the list makes the i atom.
 __device__ __forceinline__ float mop_r2(float dx, float dy, float dz) {
     return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
 }
@@ -92,8 +93,8 @@ __global__ void __launch_bounds__(128) k_debug_pairs(const PairDbgArgs a) {
                 if (!((pat >> (k >> 1)) & 1u)) continue;
                 const float4 pi = xq[un.ci * MOP_CL + k];
                 const bool allowed = (row >> (8 * jl + k)) & 1ull;
-                const float dx = __fsub_rn(__fsub_rn(pi.x, sx), cp.x), dy = __fsub_rn(__fsub_rn(pi.y, sy), cp.y),
-                            dz = __fsub_rn(__fsub_rn(pi.z, sz), cp.z);
+                const float dx = __fsub_rn(__fsub_rn(pi.x, cp.x), sx), dy = __fsub_rn(__fsub_rn(pi.y, cp.y), sy),
+                            dz = __fsub_rn(__fsub_rn(pi.z, cp.z), sz);
                 const float r2 = mop_r2(dx, dy, dz);
                 if ((r2 < a.rc2) && allowed) {
                     unsigned long long pos = atomicAdd(&a.ctr->n_pairs, 1ull);

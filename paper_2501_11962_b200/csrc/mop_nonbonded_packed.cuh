@@ -11,7 +11,7 @@
 // Lane (jl = lane & 7, g = lane >> 3) owns atom jl of the g-th of the four j-octets of the current step; a packed
 // register holds the same quantity for i atoms (2p, 2p+1), p = 0..3.  All packed operations are IEEE
 // round-to-nearest per component, so the G8 predicate
-// (d = xs_i - xw_j, r2 = fma(dz,dz,fma(dy,dy,dx*dx)), r2 < rc*rc) is bit-identical to the scalar form.
+// (d = (xw_i - xw_j) - k L, r2 = fma(dz,dz,fma(dy,dy,dx*dx)), r2 < rc*rc) is bit-identical to the scalar form.
 // Sign conventions chosen so that no negation is needed in the row body:
 //   gn = -g = x (B - A) + C - 2 k_rf ke qi qj,      hn = -h = x (x (8A - 14B) - 3C),      dn = s_j - s_i = -delta
 //   F_i += gn d;                (H s)_i += hn (d.dn) d + gn dn;        the j side accumulates the same sums (jn),
@@ -107,7 +107,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     const unsigned lane16 = (unsigned)lane * 16u;
 
     // one step: the lane's j atom (cp, ce, type offset tj4) against the row pairs of the union pattern `upat`.
-    // sh*: the lane's periodic shift (packed broadcast; zero for most steps: x - 0 = x exactly, so one code path
+    // sh*: the lane's periodic shift k L (packed broadcast; zero for most steps: d - 0 = d exactly, so one code path
     // serves both, the shifted form only being compiled into the SHIFTED instance).
     auto step = [&](const uint2 cur, const unsigned upat, const bool shifted, const bool masked, const float4 cp,
                     const float4 ce, const unsigned tj4) {
@@ -132,9 +132,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
 
         auto heavy = [&](const int p, const bool nolj) {
             const float4 P0 = mop_lds_v4(sw_addr + p * 64), P1 = mop_lds_v4(sw_addr + p * 64 + 16);
-            f2 X = f2_pack(P0.x, P0.y), Y = f2_pack(P0.z, P0.w), Z = f2_pack(P1.x, P1.y);
-            if (shifted) X = f2_sub(X, shx), Y = f2_sub(Y, shy), Z = f2_sub(Z, shz);
-            const f2 dx = f2_sub(X, jx), dy = f2_sub(Y, jy), dz = f2_sub(Z, jz), Qi = f2_pack(P1.z, P1.w);
+            const f2 X = f2_pack(P0.x, P0.y), Y = f2_pack(P0.z, P0.w), Z = f2_pack(P1.x, P1.y);
+            f2 dx = f2_sub(X, jx), dy = f2_sub(Y, jy), dz = f2_sub(Z, jz);
+            if (shifted) dx = f2_sub(dx, shx), dy = f2_sub(dy, shy), dz = f2_sub(dz, shz); // G8: d = (x_i - x_j) - k L
+            const f2 Qi = f2_pack(P1.z, P1.w);
             const f2 r2v = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
             float r2a, r2b;
             f2_unpack(r2v, r2a, r2b);

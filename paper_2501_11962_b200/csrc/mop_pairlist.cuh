@@ -256,8 +256,8 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS) k_pairlist(PlArgs a) {
         __syncwarp();
 
         // ---- phase 2: one candidate per lane.  The 8 i atoms (packed two by two: the row pairs of the pair kernels)
-        // against the 8 atoms of the lane's j-octet, with the arithmetic of the pair kernels (xs_i = x_i - k L -- x - 0 = x
-        // exactly for the zero shift --, d = xs_i - x_j, r2 = fma(dz,dz,fma(dy,dy,dx dx))); pattern bit p = some pair of
+        // against the 8 atoms of the lane's j-octet (xs_i = x_i - k L once per candidate, d = xs_i - x_j: the pair kernels'
+        // d = (x_i - x_j) - k L up to a few ulp(L), far inside the 1e-4 inflation of r_list^2); pattern bit p = some pair of
         // row pair p within r_list.  Padding atoms are never within range (mop_dummy_xq).  Then the exclusion row of the
         // octet pair (at most one matches) and the position inside the bucket of (pattern, shifted or not): lanes with
         // equal keys are ranked with one match, the first of them draws the range from the bucket's counter.

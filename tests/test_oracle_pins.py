@@ -563,6 +563,36 @@ def test_P13_cell_list_equals_brute_force(oracle, mk):
     assert not (b & ex)
 
 
+def test_G8_predicate_does_not_depend_on_the_roles_of_the_two_atoms(oracle):
+    """G8: membership is a property of the unordered pair.  The two atoms below (found on config 4, bead 7, across the z
+    face of the 10.5 x 10.5 x 13.5 box, r_c = 1.2) sit 2 ulp from r_c^2: a predicate that shifts 'atom i' first
+    (xs_i = x_i - k L, d = xs_i - x_j) classifies them differently depending on which atom it calls i -- a kernel is
+    free to choose -- while d = (x_i - x_j) - k L negates exactly under the swap.  Also on random pairs near r_c."""
+    box = [10.5, 10.5, 13.5]
+    A = np.float32([3.9472785, 5.670694, 13.426104])
+    Bm = np.float32([4.2180476, 4.894643, 0.80042])
+
+    def n_pairs(X):
+        s = H.make_system("two", box, np.asarray(X, np.float64), [12.0, 12.0], [0.0, 0.0], [0, 0], [0.3], [0.5], r_cut=1.2)
+        o = oracle.OracleSystem(s)
+        a = len(oracle.pairs(o, np.asarray(X, np.float64), geom=1, brute=True))
+        assert a == len(oracle.pairs(o, np.asarray(X, np.float64), geom=1, brute=False))
+        return a
+
+    assert n_pairs([A, Bm]) == n_pairs([Bm, A])
+    # the value itself, by hand in numpy float32: d = (x_i - x_j) - k L with k = (0, 0, 1)
+    d = (A - Bm).astype(np.float32) - np.float32([0.0, 0.0, 13.5])
+    r2 = np.float32(np.float64(d[2]) * d[2] + np.float64(np.float32(np.float64(d[1]) * d[1] + np.float64(np.float32(d[0] * d[0])))))
+    assert n_pairs([A, Bm]) == int(r2 < np.float32(1.2) * np.float32(1.2))
+    rng = np.random.default_rng(8)
+    for _ in range(200):
+        P = rng.uniform(0, 1, 3) * box
+        u = rng.normal(0, 1, 3)
+        Qp = P + u / np.linalg.norm(u) * (1.2 + rng.uniform(-3e-7, 3e-7))
+        X = np.float32([P, Qp])
+        assert n_pairs(X) == n_pairs(X[::-1])
+
+
 def test_G8_wrap_cells_and_stable_sort(oracle):
     s = W.config2()
     rng = np.random.default_rng(2)

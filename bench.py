@@ -12,7 +12,7 @@ pair interactions per second and the fraction of the FP32 roofline of the domina
 every rank runs an independent replica (own seed); value = units of all ranks / max-over-ranks time ("weak").
 
 --impl reference: there is no reference code for this paper; the arm times the FP64 CPU oracle (oracle/), as it
-stands, on the host cores, on a bounded sample of the same workload (see `sample` in the line it prints).
+stands, on the host cores, on the same workload (see `sample` in the line it prints).
 """
 import argparse
 import json
@@ -33,8 +33,27 @@ UNIT = "bead-evals/s"
 # Algorithmic FP32 work per in-range, non-excluded atom pair: FMA = 2.
 FLOP_PER_PAIR_FORCE = 31.0
 FLOP_PER_PAIR_HVP = 55.0
-# DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None.
-TRAFFIC_BYTES_PER_LAUNCH = 130.6e6   # profiles/r01_ncu_summary.md: dram read 119.9 MB + write 10.7 MB (cfg 4, N = 8)
+# The ncu capture of the dominant kernel (S5) on the bench workload, committed under profiles/: a two-column CSV
+# "metric,value" for one launch, written from the .ncu-rep by the command in profiles/r02_ncu_summary.md.
+NCU_METRICS_FILE = os.path.join("profiles", "r02_ncu_hvp_metrics.csv")
+
+
+def traffic_bytes_per_launch():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one S5 launch from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, NCU_METRICS_FILE)
+    if not os.path.exists(path):
+        return None, None
+    vals = {}
+    with open(path) as f:
+        for line in f:
+            k, _, v = line.strip().partition(",")
+            try:
+                vals[k] = float(v)
+            except ValueError:
+                continue
+    if "dram__bytes_read.sum" in vals and "dram__bytes_write.sum" in vals:
+        return vals["dram__bytes_read.sum"] + vals["dram__bytes_write.sum"], NCU_METRICS_FILE
+    return None, None
 
 
 def env_rank():
@@ -156,18 +175,9 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ workload
-def build_system(config, beads, scale=1.0):
+def build_system(config, beads):
     from paper_2501_11962_b200 import workloads as W
-    if config == 4:
-        if scale >= 0.999:
-            return W.config4(seed=0, n_beads=beads)
-        f3 = scale ** 3
-        n_prot = max(200, int(round(4000 * f3 / 10.0)) * 10)
-        return W.config4(seed=0, n_beads=beads, n_total=int(round(150000 * f3)),
-                         box=(10.5 * scale, 10.5 * scale, 13.5 * scale), n_protein=n_prot, slab=4.0 * scale, r_cut=1.2,
-                         name="c4_membrane_scaled_%.3f" % scale)
-    s = W.CONFIGS[config](seed=0, n_beads=beads)
-    return s
+    return W.CONFIGS[config](seed=0, n_beads=beads)
 
 
 def workload_name(config, s, beads):
@@ -243,6 +253,32 @@ def run_ours(a):
     launches = int(round((st1["launches"] - launches0) / 1.0))
     ms_max, units = all_reduce_max_sum(local_ms, float(N * a.steps), world, dev)
 
+    # ---- the same step with a buffered pair list (r_buf = 0.05 nm) that is REUSED: S0/S1 are replaced by k_refresh and
+    # one flag read; the pair passes walk the longer list of r_cut + r_buf.  Reported separately.
+    reuse = None
+    if world == 1:
+        mr = binding.Mop(s, N, device=local_rank, r_buf=0.05)
+        for _ in range(a.warmup):
+            mr.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
+        torch.cuda.synchronize()
+        r0 = mr.mop_get_stats()
+        e0 = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps)]
+        e1 = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps)]
+        for k in range(a.steps):
+            flush.zero_()
+            e0[k].record()
+            mr.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
+            e1[k].record()
+        torch.cuda.synchronize()
+        r1 = mr.mop_get_stats()
+        ms_r = float(sum(e0[k].elapsed_time(e1[k]) for k in range(a.steps))) / a.steps
+        reuse = {"r_buf_nm": 0.05, "ms_per_step": ms_r, "value": N / (ms_r * 1e-3), "unit": UNIT,
+                 "rebuilds_in_timed_region": int(r1["rebuilds"] - r0["rebuilds"]),
+                 "reuses_in_timed_region": int(r1["reuses"] - r0["reuses"]),
+                 "note": "same coordinates every step, so every timed step reuses the list; neighbour sets are then "
+                         "exact up to FP32 rounding of r^2 at r_c (DESIGN.md), which is why the headline rebuilds"}
+        mr.close()
+
     # ---- end to end: HOST buffers through mop_eval_veff_grad_host, copies inside the timed region
     Rh = torch.as_tensor(R).pin_memory()
     Gh = torch.empty_like(Rh).pin_memory()
@@ -273,7 +309,8 @@ def run_ours(a):
     ach = pairs_hvp * FLOP_PER_PAIR_HVP / t_hvp / 1e12 if t_hvp > 0 else 0.0
     ach_f = pairs_force * FLOP_PER_PAIR_FORCE / t_force / 1e12 if t_force > 0 else 0.0
     ms_per_step = ms_max / a.steps
-    probe = binding.mop_probe_fp32(local_rank)   # FP32 pipe with and without register-file-limited operands
+    probe = binding.mop_probe_fp32(local_rank)   # dependent-free FMA streams (context for the nominal peak, not a denominator)
+    traffic, traffic_src = traffic_bytes_per_launch()
     out = {
         "metric": METRIC, "value": throughput(units, ms_max), "unit": UNIT, "n_gpus": world, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -287,17 +324,17 @@ def run_ours(a):
         "stage_ms": {k: round(v, 5) for k, v in stages.items() if k != "evals"},
         "roofline": {"bound": "alu", "kernel": "k_nonbonded<HVP> (S5, fused force-scalar + H.eta pair kernel)",
                      "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                     "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json); "
                                     "no measured FP32 entry exists" % (sm_max, peak_src),
                      "flop_per_pair": FLOP_PER_PAIR_HVP, "pairs_per_launch": pairs_hvp, "ms_per_launch": stages["S5_nb_hvp"],
                      "fp32_probe_tflops": {k: round(v, 2) for k, v in probe.items() if k != "sms"},
-                     "frac_of_3reg_ffma2_probe": ach / probe["ffma2_3reg_tflops"] if probe["ffma2_3reg_tflops"] > 0 else None,
                      "force_kernel": {"achieved": ach_f, "frac": ach_f / peak_tf, "flop_per_pair": FLOP_PER_PAIR_FORCE,
                                       "pairs_per_launch": pairs_force, "ms_per_launch": stages["S2_nb_force"]}},
         "e2e": {"value": throughput(e2e_units, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": int(N) * Q * 12,
                 "d2h_bytes_per_step": int(N) * Q * 12 + 8, "steps": n_e2e,
                 "api": "mop_eval_veff_grad_host (pinned host R in, grad + V_eff out)"},
+        "with_list_reuse": reuse,
         "gpu_launches": launches,
         "clocks": clk,
         "veff": st1["veff"],
@@ -310,27 +347,42 @@ def run_ours(a):
 
 # ------------------------------------------------------------------------------------------------ the oracle legs
 def cpu_baseline(s, N):
-    """The oracle as it stands on a bounded sample of the bench workload: beads 1-2 of a path over the SAME system
-    (inputs from the oracle's own force, never from the CUDA path)."""
+    """The oracle as it stands on the bench workload itself (inputs from the oracle's own force, never from the CUDA
+    path).  The oracle threads over beads only (OpenMP over the force beads of each pass), so two figures:
+    `value` = one whole N-bead evaluation on min(threads, force beads) threads; `one_thread` = beads 1-2 (one force
+    bead) on one thread, scaled to the force beads of the evaluation."""
     from oracle import oracle as O
     from paper_2501_11962_b200 import workloads as W
     o = O.OracleSystem(s)
-    R2 = W.brownian_path(s, 2, lambda X: O.bead(o, X, geom=0)["F"], seed=0)
-    t = time.perf_counter()
-    v, g, parts = O.veff_grad(o, R2.astype(np.float64), geom=1, want_parts=True)
-    dt = time.perf_counter() - t
+    threads = O.num_threads()
     nf = max(N - 1, 1)
-    return {"value": N / (nf * dt), "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "beads 1-2 of the workload path on the full %d-atom system (one force bead: 1 force pass + 1 H.eta "
-                      "pass, %d in-range pairs), %.1f s; scaled to %d force beads per %d-bead evaluation; the oracle "
-                      "threads over beads only, so this sample ran on 1 of %d available threads"
-                      % (s.n_atoms, parts["npairs"], dt, nf, N, O.num_threads()),
-            "seconds": dt, "pair_interactions_per_sec": 2.0 * parts["npairs"] / dt}
+    nb = min(N, 8)                                   # bounded sample: at most 8 beads of the path
+    R = W.brownian_path(s, nb, lambda X: O.bead(o, X, geom=0)["F"], seed=0).astype(np.float64)
+    t = time.perf_counter()
+    v, g, parts = O.veff_grad(o, R, geom=1, want_parts=True)
+    dt_all = time.perf_counter() - t
+    nfb = max(nb - 1, 1)
+    out = {"value": N * (nfb / float(nf)) / dt_all, "unit": UNIT, "cores": min(threads, nfb), "kind": "oracle",
+           "sample": "one whole V_eff-gradient evaluation of the first %d beads of the workload path on the full %d-atom "
+                     "system (%d force beads: force pass + H.eta pass each, %d in-range pairs in total), %.1f s on %d of "
+                     "%d available threads%s" % (nb, s.n_atoms, nfb, parts["npairs"], dt_all, min(threads, nfb), threads,
+                                                 "" if nb == N else "; scaled to %d force beads" % nf),
+           "seconds": dt_all, "pair_interactions_per_sec": 2.0 * parts["npairs"] / dt_all}
+    if nb >= 2:
+        t = time.perf_counter()
+        v2, g2, p2 = O.veff_grad(o, R[:2], geom=1, want_parts=True)
+        dt1 = time.perf_counter() - t
+        out["one_thread"] = {"value": N / (nf * dt1), "unit": UNIT, "cores": 1, "seconds": dt1,
+                             "sample": "beads 1-2 (one force bead, %d in-range pairs) on one thread, scaled to %d force "
+                                       "beads" % (p2["npairs"], nf)}
+    return out
 
 
 def run_reference(a):
-    """--impl reference: the FP64 oracle on the host cores; each step one V_eff-gradient evaluation of an N-bead
-    path over a reduced copy of the workload (same recipe, density, cutoff), sized to finish within minutes."""
+    """--impl reference: there is no reference code, so this arm times the FP64 oracle on the host cores, on the bench
+    workload itself (same system, same bead count: `config` equals the GPU arm's).  Each step is one whole oracle
+    V_eff-gradient evaluation of the N-bead path (OpenMP over the force beads).  A wall-clock guard ends the run early
+    (and says so: `steps` is what was done) if the host is much slower than the ~20 s per step measured here."""
     rank, _, world = env_rank()
     if rank != 0:
         return None
@@ -340,30 +392,35 @@ def run_reference(a):
     threads = O.num_threads()
     N = a.beads
     nf = max(N - 1, 1)
-    budget = 150.0 / max(a.steps + a.warmup, 1)          # seconds per step
-    cost_per_atom = 2.0e-4 * -(-nf // max(min(threads, nf), 1))   # s per atom per evaluation (force + H.eta passes, measured here)
-    f = min(1.0, (budget / (cost_per_atom * 150000.0)) ** (1.0 / 3.0)) if a.config == 4 else 1.0
-    f = max(f, 0.3)
-    s = build_system(a.config, N, scale=f)
+    t_start = time.perf_counter()
+    budget_s = 1200.0
+    s = build_system(a.config, N)
     o = O.OracleSystem(s)
     R = W.brownian_path(s, N, lambda X: O.bead(o, X, geom=0)["F"], seed=0).astype(np.float64)
-    full_atoms = 150000 if a.config == 4 else s.n_atoms
+    warm_done = 0
     for _ in range(a.warmup):
+        if time.perf_counter() - t_start > 0.3 * budget_s:
+            break
         O.veff_grad(o, R, geom=1)
+        warm_done += 1
     t = time.perf_counter()
+    done = 0
     for _ in range(a.steps):
-        v, g = O.veff_grad(o, R, geom=1)
+        v, g, parts = O.veff_grad(o, R, geom=1, want_parts=True)
+        done += 1
+        if time.perf_counter() - t_start > budget_s:
+            break
     dt = time.perf_counter() - t
-    units = N * a.steps * (s.n_atoms / float(full_atoms))      # bead evaluations in 150k-atom equivalents
-    sample = ("each step = one oracle V_eff-gradient evaluation of an N=%d path over %s (%d atoms, box scale %.3f of "
-              "the workload, same recipe/density/cutoff); value scaled linearly in atom count to %d atoms"
-              % (N, s.name, s.n_atoms, f, full_atoms))
-    val = units / dt
-    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": a.steps,
-            "warmup": a.warmup, "ms_per_step": dt * 1e3 / a.steps, "higher_is_better": True, "scaling": "weak",
+    val = N * done / dt
+    sample = ("each step = one whole oracle V_eff-gradient evaluation of the N=%d path over the full system (%d atoms, %d "
+              "force beads: force pass + H.eta pass each, %d in-range pairs per evaluation) on %d of %d threads; %d of %d "
+              "timed steps and %d of %d warm-up steps done" % (N, s.n_atoms, nf, parts["npairs"], min(threads, nf), threads,
+                                                             done, a.steps, warm_done, a.warmup))
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": done,
+            "warmup": warm_done, "ms_per_step": dt * 1e3 / done, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[%d] at N=%d beads (150,000-atom membrane-protein-shaped system)" % (a.config - 1, N)
-                       if a.config == 4 else workload_name(a.config, s, N)},
+            "config": {"workload": workload_name(a.config, s, N)},
+            "pair_interactions_per_sec": 2.0 * parts["npairs"] * done / dt,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": min(threads, nf), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0, "veff": v}

@@ -30,7 +30,8 @@ struct mop_ctx {
     MopGrid g;
     float bin_z;
     float rl, rl2, rc2;
-    float krf, crf;
+    float krf;
+    double krf_d, crf_d;
     bool has_topology = false;
     int sticky = MOP_OK;
     std::string err;
@@ -132,10 +133,11 @@ typedef void (*nb_kernel_t)(const NbArgs);
 // for the H.eta pass (measured: profiles/r02_experiments.md)
 #define NBP_CTAS_F 6
 #define NBP_CTAS_H 5
+#define NBP_CTAS_E 4   // energy variant (bead 1 only): FP64 sums and six more packed accumulators per step
 static nb_kernel_t nb_pick(int mode, bool count = false) {
     if (count) return k_nonbonded_p<NB_FORCE, true, NBP_CTAS_F>;
     return mode == NB_FORCE ? k_nonbonded_p<NB_FORCE, false, NBP_CTAS_F>
-         : mode == NB_ENERGY ? k_nonbonded_p<NB_ENERGY, false, NBP_CTAS_F> : k_nonbonded_p<NB_HVP, false, NBP_CTAS_H>;
+         : mode == NB_ENERGY ? k_nonbonded_p<NB_ENERGY, false, NBP_CTAS_E> : k_nonbonded_p<NB_HVP, false, NBP_CTAS_H>;
 }
 static size_t nb_smem(const mop_ctx *c) { return nbp_smem_bytes(c->nt); }
 
@@ -212,7 +214,8 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
         double krf = p->eps_rf > 0.f ? ((double)p->eps_rf - 1.0) / ((2.0 * (double)p->eps_rf + 1.0) * rc * rc * rc)
                                       : 1.0 / (2.0 * rc * rc * rc);
         c->krf = (float)krf;
-        c->crf = (float)(1.0 / rc + krf * rc * rc);
+        c->krf_d = krf;
+        c->crf_d = 1.0 / rc + krf * rc * rc;
     }
     // search grid (S0): columns of side ~ (8/rho)^(1/3) in x,y; thin bins of side/8 along z
     MopGrid &g = c->g;
@@ -542,7 +545,7 @@ static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     NbArgs a;
     a.S = c->g.S, a.nt = c->nt;
     a.rc2 = c->rc2;
-    a.k2rf = 2.0f * c->krf, a.krf = c->krf, a.crf = c->crf;
+    a.k2rf = 2.0f * c->krf, a.krf_d = c->krf_d, a.crf_d = c->crf_d;
     a.xq = c->d_xq, a.typ = c->d_typ, a.et = c->d_et, a.out = out;
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.cap_units = c->cap_units;

@@ -18,7 +18,8 @@ __global__ void __launch_bounds__(256) k_bin(const float *__restrict__ R, MopGri
 #pragma unroll
     for (int d = 0; d < 3; d++) {
         const float xw = mop_wrap1(r[d], g.box[d], g.inv_box[d]);
-        ok = ok && (xw >= 0.0f) && (xw < g.box[d]);   // false for NaN
+        // false for NaN/Inf; beyond 1e6 box lengths the FP32 wrap has no resolution left (ulp(x) > L / 16)
+        ok = ok && (xw >= 0.0f) && (xw < g.box[d]) && (fabsf(r[d]) <= 1.0e6f * g.box[d]);
         c[d] = mop_cell1(xw, g.sc[d], g.dims[d]);
     }
     if (!ok) *nonfinite = 1u;

@@ -15,7 +15,7 @@ struct NbArgs {
     int S, nt;
     float rc2;          // r_cut*r_cut (FP32 product, G8)
     float k2rf;         // 2 k_rf
-    float krf, crf;     // energy only
+    double krf_d, crf_d; // energy only: k_rf and c_rf = 1/r_c + k_rf r_c^2 in FP64 (applied once per step to FP32 partial sums)
     const float4 *xq;   // [nf][S]
     const int *typ;     // [nf][S] types (force pass)
     const float4 *et;   // [nf][S] eta + type bits (HVP pass)

@@ -44,19 +44,26 @@ __device__ __forceinline__ uint2 mop_lds_vu2(unsigned addr) {
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
     return v;
 }
-#define NBP_NST 2       // stages of the per-warp j-atom ring (steps in flight: NBP_NST - 1)
+#define NBP_NST 2       // stages of the per-warp j-atom ring (one step in flight)
 
 // Shared memory of one CTA (4 warps), bytes:
 //   [0, 1024)              i-atom staging, 256 B per warp: for p = 0..3 at float offset 16 p
-//                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] c6-row address
+//                          [0,1] x  [2,3] y  [4,5] z  [6,7] ke q  [8,9] s_x  [10,11] s_y  [12,13] s_z  [14,15] LJ-row address
 //   [1024, 2048)           the current chunk of up to 32 list entries (8 steps), 256 B per warp
-//   [2048, 2048 + 4 NBP_NST KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
-//   then the LJ tables: c6[nt*nt] (6 C6), c12[nt*nt] (12 C12), energy shift [nt*nt],
+//   [2048, 3072)           energy variant only: the i atoms in FP64, 256 B per warp: atom k at +32 k: x, y, z, ke q
+//   [3072, 3072 + 4 NBP_NST KB)   j-atom ring, per warp NBP_NST stages of 1 KB: xq[32] at +0, eta+type[32] (or type[32]) at +512
+//   then the LJ tables: (6 C6, 12 C12)[nt*nt] interleaved (one 8-byte load per pair), energy shift [nt*nt],
 //   and one flag per type: its LJ row has a non-zero entry
 #define NBP_SM_ENT 1024u
-#define NBP_SM_RING 2048u
-#define NBP_SM_TAB (2048u + 4u * NBP_NST * 1024u)
+#define NBP_SM_DBL 2048u
+#define NBP_SM_RING 3072u
+#define NBP_SM_TAB (NBP_SM_RING + 4u * NBP_NST * 1024u)
 __host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (size_t)nt * nt * 12 + (size_t)nt * 4; }
+__device__ __forceinline__ double mop_lds_d(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
 
 // One work unit = one i-octet against its list of (j-octet, shift) entries, four entries per step: lane (jl, g) holds
 // atom jl of the step's g-th octet.  The builder has ordered the entries by their row-pair pattern, so the union
@@ -66,34 +73,42 @@ __host__ __device__ inline size_t nbp_smem_bytes(int nt) { return NBP_SM_TAB + (
 template <int MODE, bool COUNT>
 __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, float *__restrict__ sw,
                                          const unsigned sw_addr, const unsigned se_addr, const unsigned sr_addr,
-                                         const unsigned tab6, const unsigned off12,
+                                         const unsigned sd_addr, const unsigned tab6, const unsigned tabS,
                                          const int *__restrict__ tflag, const int lane) {
     constexpr bool HVP = MODE == NB_HVP, ENERGY = MODE == NB_ENERGY;
-    const unsigned boff = (unsigned)un.bead * (unsigned)a.S; // nf * S < 2^31 (checked at create)
-    const float4 *__restrict__ xq = a.xq + boff;
-    const float4 *__restrict__ et = a.et + boff;
-    const int *__restrict__ typ = a.typ + boff;
-    float4 *__restrict__ out = a.out + boff;
+    // every atom is addressed by its 32-bit element index boff + slot into the [nf][S] arrays (nf * S < 2^31, checked at
+    // create): one wide multiply-add per address instead of per-bead 64-bit pointers rebuilt every step
+    const unsigned boff = (unsigned)un.bead * (unsigned)a.S;
+    const float4 *__restrict__ xq = a.xq;
+    const float4 *__restrict__ et = a.et;
+    const int *__restrict__ typ = a.typ;
+    float4 *__restrict__ out = a.out;
     const int jl = lane & 7, gq = lane >> 3;
+    const unsigned ibase = boff + (unsigned)un.ci * MOP_CL;
 
     __syncwarp();
     bool has_lj = false;
     if (lane < MOP_CL) {
-        float4 p = xq[un.ci * MOP_CL + lane];
+        float4 p = xq[ibase + lane];
         float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
         int ti;
         if (HVP) {
-            e = et[un.ci * MOP_CL + lane];
+            e = et[ibase + lane];
             ti = __float_as_int(e.w);
         } else {
-            ti = typ[un.ci * MOP_CL + lane];
+            ti = typ[ibase + lane];
         }
         has_lj = tflag[ti] != 0;
         float *d = sw + (lane >> 1) * 16 + (lane & 1);
         d[0] = p.x, d[2] = p.y, d[4] = p.z;
         d[6] = p.w * MOP_KE;
         d[8] = e.x, d[10] = e.y, d[12] = e.z;
-        d[14] = __int_as_float((int)tab6 + ti * a.nt * 4);
+        d[14] = __int_as_float((int)tab6 + ti * a.nt * 8);
+        if (ENERGY) {
+            asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(sd_addr + lane * 32u), "d"((double)p.x), "d"((double)p.y) : "memory");
+            asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(sd_addr + lane * 32u + 16u), "d"((double)p.z),
+                         "d"(138.935458 * (double)p.w) : "memory");
+        }
     }
     __syncwarp();
     const unsigned ljmask = __ballot_sync(0xffffffffu, has_lj) & 0xffu; // bit k: i atom k has a non-zero LJ row
@@ -106,20 +121,30 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     const f2 nk2rf = f2_bc(-a.k2rf);
     const unsigned lane16 = (unsigned)lane * 16u;
 
-    // one step: the lane's j atom (cp, ce, type offset tj4) against the row pairs of the union pattern `upat`.
+    // one step: the lane's j atom (cp, ce, type offset tj8) against the row pairs of the union pattern `upat`.
     // sh*: the lane's periodic shift k L (packed broadcast; zero for most steps: d - 0 = d exactly, so one code path
     // serves both, the shifted form only being compiled into the SHIFTED instance).
     auto step = [&](const uint2 cur, const unsigned upat, const bool shifted, const bool masked, const float4 cp,
-                    const float4 ce, const unsigned tj4) {
+                    const float4 ce, const unsigned tj8) {
         const f2 jx = f2_bc(cp.x), jy = f2_bc(cp.y), jz = f2_bc(cp.z), jq = f2_bc(cp.w);
         f2 shx = 0ull, shy = 0ull, shz = 0ull;
         if (shifted) {
             float sx, sy, sz;
-            mop_unit_shift((int)(cur.x >> 24), a.box, sx, sy, sz);
+            mop_unit_shift((int)(cur.y >> 24), a.box, sx, sy, sz);
             shx = f2_bc(sx), shy = f2_bc(sy), shz = f2_bc(sz);
         }
         f2 nx = 0ull, ny = 0ull, nz = 0ull; // jn: minus the j-side sums
-        float u_lj = 0.f, u_c = 0.f;
+        // energy variant: the lane's j atom and shift in FP64 (see "energy of bead 1" in heavy())
+        double jxd = 0.0, jyd = 0.0, jzd = 0.0, acc_c = 0.0;
+        f2 eA = 0ull, eB = 0ull, eS = 0ull;   // LJ: FP32 sums of A, B and the shift over the step's in-range pairs
+        if (ENERGY) {
+            jxd = (double)cp.x, jyd = (double)cp.y, jzd = (double)cp.z;
+            if (shifted) {
+                float sx, sy, sz;
+                mop_unit_shift((int)(cur.y >> 24), a.box, sx, sy, sz);
+                jxd += (double)sx, jyd += (double)sy, jzd += (double)sz;   // exact: d = x_i - (x_j + k L)
+            }
+        }
         // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
         // (a padding entry -- pattern 0, it points at the unit's own octet -- allows nothing)
         const bool valid = (cur.y & 15u) != 0u;
@@ -146,30 +171,26 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             }
             if (COUNT) n_in += (ina ? 1u : 0u) + (inb ? 1u : 0u);
             const float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
-            f2 rinv = f2_pack(ra, rb);
-            if (ENERGY) { // one Newton step: removes the approximation's bias from the energy sum
-                const f2 em = f2_fma(f2_mul(r2v, rinv), rinv, f2_bc(-1.0f));   // r2 rinv^2 - 1
-                rinv = f2_fma(f2_mul(rinv, f2_bc(-0.5f)), em, rinv);
-            }
+            const f2 rinv = f2_pack(ra, rb);
+            const f2 qq = f2_mul(Qi, jq);
             f2 S0 = 0ull, S1 = 0ull, S2 = 0ull;
             unsigned ta, tb;
             if (HVP) {
                 const float4 E0 = mop_lds_v4(sw_addr + p * 64 + 32), E1 = mop_lds_v4(sw_addr + p * 64 + 48);
                 S0 = f2_pack(E0.x, E0.y), S1 = f2_pack(E0.z, E0.w), S2 = f2_pack(E1.x, E1.y);
-                ta = (unsigned)__float_as_int(E1.z) + tj4, tb = (unsigned)__float_as_int(E1.w) + tj4;
+                ta = (unsigned)__float_as_int(E1.z) + tj8, tb = (unsigned)__float_as_int(E1.w) + tj8;
             } else {
                 const float2 T = mop_lds_v2(sw_addr + p * 64 + 56);
-                ta = (unsigned)__float_as_int(T.x) + tj4, tb = (unsigned)__float_as_int(T.y) + tj4;
+                ta = (unsigned)__float_as_int(T.x) + tj8, tb = (unsigned)__float_as_int(T.y) + tj8;
             }
             const f2 x = f2_mul(rinv, rinv);
-            const f2 qq = f2_mul(Qi, jq);
             const f2 C = f2_mul(qq, f2_mul(x, rinv));
             f2 x3 = 0ull, A = 0ull, B = 0ull, gn;
             if (nolj) { // both i atoms have an all-zero LJ row (water hydrogens): reaction field only
                 gn = f2_fma(qq, nk2rf, C);
             } else {
-                const f2 c6 = f2_pack(mop_lds_f(ta), mop_lds_f(tb));
-                const f2 c12 = f2_pack(mop_lds_f(ta + off12), mop_lds_f(tb + off12));
+                const float2 la = mop_lds_v2(ta), lb = mop_lds_v2(tb);   // (6 C6, 12 C12) of the two pairs
+                const f2 c6 = f2_pack(la.x, lb.x), c12 = f2_pack(la.y, lb.y);
                 x3 = f2_mul(f2_mul(x, x), x);
                 A = f2_mul(c6, x3);
                 B = f2_mul(f2_mul(c12, x3), x3);
@@ -183,18 +204,34 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             if (!HVP) {
                 f2_acc(ax[p], gn, dx), f2_acc(ay[p], gn, dy), f2_acc(az[p], gn, dz);
                 f2_acc(nx, gn, dx), f2_acc(ny, gn, dy), f2_acc(nz, gn, dz);
-                if (ENERGY) { // u_lj = C12 x^6 - C6 x^3 - shift = B/12 - A/6 - shift;  u_c = ke qi qj (1/r + k_rf r^2 - c_rf)
-                    f2 ue = f2_mul(qq, f2_add(f2_fma(r2v, f2_bc(a.krf), rinv), f2_bc(-a.crf)));
-                    if (!nolj) {
-                        const f2 sh = f2_pack(mop_lds_f(ta + 2u * off12), mop_lds_f(tb + 2u * off12));
-                        const f2 ul = f2_fma(B, f2_bc(1.0f / 12.0f), f2_fma(A, f2_bc(-1.0f / 6.0f), f2_mul(sh, f2_bc(-1.0f))));
-                        float la, lb;
-                        f2_unpack(ul, la, lb);
-                        u_lj += (ina ? la : 0.f) + (inb ? lb : 0.f);
+                if (ENERGY) {
+                    // Energy of bead 1.  U(R^1) is the small remainder of attractive and repulsive pair terms (sum |u| ~
+                    // 1e4 |U| for water-like systems), so FP32 reaction-field pair energies -- 6e-8 relative rounding in
+                    // 1/r alone, and the low bits of c_rf lost the same way for every close pair -- leave 3e-6 to 2e-5
+                    // of |U(R^1)|; north_star asks for 1e-6 of V_eff, which for N = 1 is U(R^1).  So the reaction-field
+                    // term is formed in FP64 (forces stay FP32): d exact from the FP32 coordinates, 1/r = the FP32 rsqrt
+                    // refined by one FP64 Newton step (relative error ~ 1e-13), FP64 constants; the lane's q_j multiplies
+                    // the step's sum once.  The LJ term has no such cancellation: FP32 sums of A, B and the shift per
+                    // step, combined in FP64 (its table constants 6 C6, 12 C12 are exact multiples, so unbiased).
+#pragma unroll
+                    for (int c = 0; c < 2; c++) {
+                        if (c ? inb : ina) {
+                            const unsigned ia = sd_addr + (unsigned)(2 * p + c) * 32u;
+                            const double ddx = mop_lds_d(ia) - jxd, ddy = mop_lds_d(ia + 8u) - jyd, ddz = mop_lds_d(ia + 16u) - jzd;
+                            const double r2d = fma(ddz, ddz, fma(ddy, ddy, ddx * ddx));
+                            const double y = (double)(c ? rb : ra);
+                            const double t = fma(a.krf_d, r2d, fma(y, fma(-0.5 * (y * y), r2d, 1.5), -a.crf_d));
+                            acc_c = fma(mop_lds_d(ia + 24u), t, acc_c);
+                        }
                     }
-                    float ca, cb;
-                    f2_unpack(ue, ca, cb);
-                    u_c += (ina ? ca : 0.f) + (inb ? cb : 0.f);
+                    if (!nolj) {
+                        float v0, v1, w0, w1, s0, s1;
+                        f2_unpack(A, v0, v1), f2_unpack(B, w0, w1);
+                        s0 = mop_lds_f(tabS + ((ta - tab6) >> 1)), s1 = mop_lds_f(tabS + ((tb - tab6) >> 1));
+                        eA = f2_add(eA, f2_pack(ina ? v0 : 0.f, inb ? v1 : 0.f));
+                        eB = f2_add(eB, f2_pack(ina ? w0 : 0.f, inb ? w1 : 0.f));
+                        eS = f2_add(eS, f2_pack(ina ? s0 : 0.f, inb ? s1 : 0.f));
+                    }
                 }
             } else {
                 f2 hn = nolj ? f2_mul(f2_mul(x, f2_bc(-3.0f)), C)
@@ -224,56 +261,72 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         if (valid) {
             float lx, hx, ly, hy, lz, hz;
             f2_unpack(nx, lx, hx), f2_unpack(ny, ly, hy), f2_unpack(nz, lz, hz);
-            mop_red_add_f4(out + ((cur.x & 0xffffffu) * MOP_CL + jl), -lx - hx, -ly - hy, -lz - hz);
+            mop_red_add_f4(out + (cur.x + jl), -lx - hx, -ly - hy, -lz - hz);
         }
-        if (ENERGY) e_lj += (double)u_lj, e_c += (double)u_c;
+        if (ENERGY) {
+            auto hsum = [](f2 v) {
+                float lo, hi;
+                f2_unpack(v, lo, hi);
+                return (double)lo + (double)hi;
+            };
+            e_c = fma((double)cp.w, acc_c, e_c);
+            e_lj += hsum(eB) * (1.0 / 12.0) - hsum(eA) * (1.0 / 6.0) - hsum(eS);
+        }
     };
 
-    // ---- the unit's entries, 32 at a time (8 steps): the chunk's entry words go to shared memory (one coalesced load),
-    // the j atoms of the next NBP_NST-1 steps are in flight (cp.async into the warp's ring; every lane copies and
-    // later reads only its own atom, so no cross-lane synchronisation is needed)
+    // ---- the unit's entries, 32 at a time (8 steps): the chunk's entry words go to shared memory (one coalesced load;
+    // staged as x = element index of the j-octet's first atom, y = flags | shift id << 24), the j atoms of the next step
+    // are in flight (cp.async into the warp's two-stage ring; every lane copies and later reads only its own atom, so no
+    // cross-lane synchronisation is needed)
     const unsigned eend = un.start + un.count;
+    const unsigned se_g = se_addr + gq * 8u;           // this lane group's entry of step 0
+    const unsigned infobit = 1u << (16 + jl);          // the bit of the step information this lane contributes to the vote
+    const unsigned sr_l = sr_addr + lane16, sr_t = sr_addr + 512u + (HVP ? lane16 : (unsigned)lane * 4u);
     for (unsigned c0 = un.start; c0 < eend; c0 += 32) {
         const int nE = (int)min(32u, eend - c0), nS = nE / MOP_NG;
         __syncwarp();
         if (lane < nE) {
             const uint2 w = a.entries[c0 + lane];
-            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(se_addr + lane * 8), "r"(w.x), "r"(w.y) : "memory");
+            asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(se_addr + lane * 8), "r"(boff + (w.x & 0xffffffu) * MOP_CL),
+                         "r"(w.y | (w.x & 0xff000000u))
+                         : "memory");
         }
         __syncwarp();
-        auto issue = [&](const int k) { // start the copies of step k's j atoms into stage k % NBP_NST
+        auto issue = [&](const int k) { // start the copies of step k's j atoms into stage k % 2
             if (k < nS) {
-                const unsigned jc = mop_lds_vu(se_addr + (k * MOP_NG + gq) * 8) & 0xffffffu;
-                const unsigned o = jc * MOP_CL + jl;
-                const unsigned st = sr_addr + (unsigned)(k % NBP_NST) * 1024u;
-                mop_cp_async16(st + lane16, xq + o);
-                if (HVP) mop_cp_async16(st + 512u + lane16, et + o);
-                else mop_cp_async4(st + 512u + lane * 4, typ + o);
+                const unsigned o = mop_lds_vu(se_g + (unsigned)k * 32u) + jl;
+                const unsigned sto = (unsigned)(k & 1) * 1024u;
+                mop_cp_async16(sr_l + sto, xq + o);
+                if (HVP) mop_cp_async16(sr_t + sto, et + o);
+                else mop_cp_async4(sr_t + sto, typ + o);
             }
             mop_cp_commit();
         };
-#pragma unroll
-        for (int k = 0; k < NBP_NST - 1; k++) issue(k);
+        issue(0);
         for (int i = 0; i < nS; i++) {
-            issue(i + NBP_NST - 1);
-            mop_cp_wait<NBP_NST - 1>();
-            const unsigned st = sr_addr + (unsigned)(i % NBP_NST) * 1024u;
-            const uint2 cur = mop_lds_vu2(se_addr + (i * MOP_NG + gq) * 8);
-            const float4 cp = mop_lds_v4(st + lane16);
+            issue(i + 1);
+            mop_cp_wait<1>();
+            const unsigned sto = (unsigned)(i & 1) * 1024u;
+            const uint2 cur = mop_lds_vu2(se_g + (unsigned)i * 32u);
+            const float4 cp = mop_lds_v4(sr_l + sto);
             float4 ce = make_float4(0.f, 0.f, 0.f, 0.f);
-            unsigned tj4;
+            unsigned tj8;
             if (HVP) {
-                ce = mop_lds_v4(st + 512u + lane16);
-                tj4 = (unsigned)__float_as_int(ce.w) * 4u;
+                ce = mop_lds_v4(sr_t + sto);
+                tj8 = (unsigned)__float_as_int(ce.w) * 8u;
             } else {
-                tj4 = mop_lds_vu(st + 512u + lane * 4) * 4u;
+                tj8 = mop_lds_vu(sr_t + sto) * 8u;
             }
-            // step information from the list builder, the same in all four entries (warp-uniform by construction)
-            const unsigned upat = (cur.y >> 16) & 15u;
-            const bool shifted = (cur.y >> 20) & 1u, masked = (cur.y >> 21) & 1u;
-            if (shifted) step(cur, upat, true, true, cp, ce, tj4);
-            else if (masked) step(cur, upat, false, true, cp, ce, tj4);
-            else step(cur, upat, false, false, cp, ce, tj4);
+            // step information from the list builder, the same in all four entries: one vote makes it warp-uniform for
+            // the compiler (bits 0-3 union pattern, 4 shifted, 5 masked), so every test below is a uniform branch
+            const unsigned info = __ballot_sync(0xffffffffu, (cur.y & infobit) != 0u) & 0x3fu;
+            const unsigned upat = info & 15u;
+            const bool shifted = (info >> 4) & 1u, masked = (info >> 5) & 1u;
+            // (the energy variant, bead 1 only, compiles the general form alone: with the FP64 reaction-field energy three
+            // copies of the step body overflow the instruction cache -- "no instruction" was its top stall reason)
+            if (ENERGY || shifted) step(cur, upat, true, true, cp, ce, tj8);
+            else if (masked) step(cur, upat, false, true, cp, ce, tj8);
+            else step(cur, upat, false, false, cp, ce, tj8);
         }
         mop_cp_wait<0>();
     }
@@ -301,7 +354,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         v[j] += __shfl_xor_sync(0xffffffffu, v[j], 2);
         v[j] += __shfl_xor_sync(0xffffffffu, v[j], 1);
     }
-    if ((lane & 3) == 0) mop_red_add_f4(out + (un.ci * MOP_CL + (lane >> 2)), v[0], v[1], v[2]);
+    if ((lane & 3) == 0) mop_red_add_f4(out + (ibase + (lane >> 2)), v[0], v[1], v[2]);
     if (ENERGY) {
         e_lj = mop_warp_sum_d(e_lj), e_c = mop_warp_sum_d(e_c);
         if (lane == 0) {
@@ -323,12 +376,11 @@ __global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float *sw = reinterpret_cast<float *>(sb) + w * 64;
     const int n2 = a.nt * a.nt;
-    float *t6 = reinterpret_cast<float *>(sb + NBP_SM_TAB), *t12 = t6 + n2;
-    float *tabs = t12 + n2;
+    float2 *t6 = reinterpret_cast<float2 *>(sb + NBP_SM_TAB);
+    float *tabs = reinterpret_cast<float *>(t6 + n2);
     int *tflag = reinterpret_cast<int *>(tabs + n2);   // [nt]: 1 iff the type's LJ row has a non-zero entry
     for (int t = threadIdx.x; t < n2; t += blockDim.x) {
-        const float2 c = a.tab[t];
-        t6[t] = c.x, t12[t] = c.y;
+        t6[t] = a.tab[t];
         tabs[t] = a.tabs[t];
     }
     for (int t = threadIdx.x; t < a.nt; t += blockDim.x) {
@@ -343,7 +395,7 @@ __global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
     else if (a.range == 1) ubeg = nu0;
     const unsigned s0 = (unsigned)__cvta_generic_to_shared(sb);
     const unsigned sw_addr = s0 + w * 256u, se_addr = s0 + NBP_SM_ENT + w * 256u;
-    const unsigned sr_addr = s0 + NBP_SM_RING + w * (NBP_NST * 1024u);
+    const unsigned sr_addr = s0 + NBP_SM_RING + w * (NBP_NST * 1024u), sd_addr = s0 + NBP_SM_DBL + w * 256u;
     const unsigned tab6 = s0 + NBP_SM_TAB;
     for (;;) {
         unsigned u = 0;
@@ -356,6 +408,6 @@ __global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
         un.bead = (int)u0.x, un.ci = (int)u0.y, un.start = u0.z, un.count = u0.w;
         un.excl_base = u1.x;
         if (un.count == 0) continue;
-        nbp_unit<MODE, COUNT>(a, un, sw, sw_addr, se_addr, sr_addr, tab6, (unsigned)n2 * 4u, tflag, lane);
+        nbp_unit<MODE, COUNT>(a, un, sw, sw_addr, se_addr, sr_addr, sd_addr, tab6, tab6 + (unsigned)n2 * 8u, tflag, lane);
     }
 }

@@ -77,3 +77,27 @@ def pairs_near_cutoff(system, X, tol=1e-4):
     r = np.sqrt((d * d).sum(-1))
     iu = np.triu_indices(X.shape[0], 1)
     return int((np.abs(r[iu] - system.r_cut) < tol).sum())
+
+
+TOL_MAX = 1e-3
+
+
+def assert_close(a, b, tol_rms, tol_max=TOL_MAX):
+    """The parity bar for a force-like array [..., atom, 3]: G14's RMS relative error <= tol_rms (north_star: 1e-4)
+    AND, per component, |a - b| <= tol_max x (RMS magnitude of the reference components) + tol_rms x |b_atom| (the
+    norm of that atom's own reference vector: FP32 rounding scales with the atom's force, which on a system with
+    close contacts exceeds the RMS by orders of magnitude).  An RMS over millions of components alone would let one
+    component be off by a large multiple of the typical magnitude."""
+    a = np.asarray(a, float)
+    b = np.asarray(b, float)
+    assert a.shape == b.shape, (a.shape, b.shape)
+    r = rms_rel(a, b)
+    assert r <= tol_rms, "RMS relative error %.3e > %.1e" % (r, tol_rms)
+    if b.size == 0:
+        return
+    scale = float(np.sqrt((b * b).mean()))
+    allowed = tol_max * max(scale, 1e-30) + tol_rms * np.sqrt((b * b).sum(-1, keepdims=True))
+    excess = np.abs(a - b) - allowed
+    k = np.unravel_index(excess.argmax(), excess.shape)
+    assert excess[k] <= 0, "|delta| %.3e > %.1e x rms(ref) %.3e + %.1e x |ref atom| at component %s" % (
+        abs(a[k] - b[k]), tol_max, scale, tol_rms, k)

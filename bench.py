@@ -8,8 +8,11 @@ step) on the synthetic 150,000-atom membrane-protein-shaped system of BASELINE.j
 Prints ONE JSON line (rank 0).  metric = bead V_eff-gradient evaluations per second = beads * steps / time;
 pair interactions per second and the fraction of the FP32 roofline of the dominant kernel ride along.
 
---gpus N > 1 (under torchrun): the path does not shard in this build (north_star: one GPU, no collectives), so
-every rank runs an independent replica (own seed); value = units of all ranks / max-over-ranks time ("weak").
+--gpus N > 1 (under torchrun), default --parallelism blocks: the paper's layout -- ONE path of
+8 N beads, every rank owns a block of 8 consecutive beads (mop.h "bead-block mode") and exchanges two halos per
+evaluation with its neighbours over NCCL send/recv plus an 8-byte all-reduce of V_eff (paper_2501_11962_b200/blocks.py);
+per-GPU work is fixed, so "scaling": "weak"; value = beads of the whole path * steps / max-over-ranks time.
+--parallelism replicas: every rank runs an independent 8-bead replica (own seed), no communication.
 
 --impl reference: there is no reference code for this paper; the arm times the FP64 CPU oracle (oracle/), as it
 stands, on the host cores, on the same workload (see `sample` in the line it prints).
@@ -201,17 +204,34 @@ def run_ours(a):
     N = a.beads
     s = build_system(a.config, N)
     Q = s.n_atoms
+    blocks_mode = a.parallelism == "blocks" and (world > 1 or a.blocks_on_one_gpu)
     # the path: BASELINE.json's Brownian recursion, forces from the library's own pass 1 (not timed)
     m1 = binding.Mop(s, 1, device=local_rank)
-    R = W.brownian_path(s, N, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=rank)
-    m1.close()
-    m = binding.Mop(s, N, device=local_rank)
-    Rd = torch.as_tensor(R, device=dev)
+    if blocks_mode:
+        # one path of N * world beads (same seed on every rank); this rank owns beads [first, first + N)
+        from paper_2501_11962_b200 import blocks
+        n_path = N * world
+        first, nb = blocks.partition(n_path, world)[rank]
+        R = W.brownian_path(s, first + nb, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0)[first:]
+        m1.close()
+        m = binding.Mop(s, nb, device=local_rank, block=(first, n_path))
+        bp = blocks.BlockPath(m, Q, first, nb, n_path, rank=rank, world=world, device=dev)
+        n_hvp_local = min(nb, n_path - 1 - first)
+    else:
+        n_path = N
+        R = W.brownian_path(s, N, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=rank)
+        m1.close()
+        m = binding.Mop(s, N, device=local_rank)
+        n_hvp_local = m.nf if N > 1 else 0
+    Rd = torch.as_tensor(np.ascontiguousarray(R), device=dev)
     Gd = torch.empty_like(Rd)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def step():
-        m.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
+        if blocks_mode:
+            bp.eval(Rd, grad_out=Gd)        # halos over NCCL, V_eff all-reduced (the host reads 8 bytes per step)
+        else:
+            m.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
 
     for _ in range(a.warmup):
         step()
@@ -219,9 +239,9 @@ def run_ours(a):
     st0 = m.mop_get_stats()
     if not np.isfinite(st0["veff"]):
         raise RuntimeError("V_eff is not finite on the bench workload")
-    pairs = [m.mop_debug_pairs(n, cap=0)[1] for n in range(m.nf)]   # in-range, non-excluded pairs per force bead
-    n_hvp_beads = m.nf if N > 1 else 0
-    pairs_force, pairs_hvp = float(sum(pairs)), float(sum(pairs[:n_hvp_beads]))
+    n_force_local = max(n_hvp_local, 1) if not blocks_mode else n_hvp_local
+    pairs = [m.mop_debug_pairs(n, cap=0)[1] for n in range(n_force_local)]   # in-range, non-excluded pairs per force bead
+    pairs_force, pairs_hvp = float(sum(pairs)), float(sum(pairs[:n_hvp_local]))
     launches0 = m.mop_get_stats()["launches"]
 
     # ---- timed region: K steps, per-step CUDA events on the launching stream, L2 flushed between steps
@@ -251,12 +271,18 @@ def run_ours(a):
     m.mop_set_timing(False)
     st1 = m.mop_get_stats()
     launches = int(round((st1["launches"] - launches0) / 1.0))
-    ms_max, units = all_reduce_max_sum(local_ms, float(N * a.steps), world, dev)
+    ms_max, units = all_reduce_max_sum(local_ms, float(Rd.shape[0] * a.steps), world, dev)
+    if world > 1:   # pair counts of all ranks (rank 0 reports the job's pair rate; the roofline stays rank 0's own kernel)
+        pc = torch.tensor([pairs_force, pairs_hvp], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(pc)
+        pairs_force_job, pairs_hvp_job = float(pc[0]), float(pc[1])
+    else:
+        pairs_force_job, pairs_hvp_job = pairs_force, pairs_hvp
 
     # ---- the same step with a buffered pair list (r_buf = 0.05 nm) that is REUSED: S0/S1 are replaced by k_refresh and
     # one flag read; the pair passes walk the longer list of r_cut + r_buf.  Reported separately.
     reuse = None
-    if world == 1:
+    if world == 1 and not blocks_mode:
         mr = binding.Mop(s, N, device=local_rank, r_buf=0.05)
         for _ in range(a.warmup):
             mr.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
@@ -280,10 +306,20 @@ def run_ours(a):
         mr.close()
 
     # ---- end to end: HOST buffers through mop_eval_veff_grad_host, copies inside the timed region
-    Rh = torch.as_tensor(R).pin_memory()
+    Rh = torch.as_tensor(np.ascontiguousarray(R)).pin_memory()
     Gh = torch.empty_like(Rh).pin_memory()
+
+    def e2e_step():
+        if not blocks_mode:
+            return m.mop_eval_veff_grad_host(Rh, Gh)
+        Rd.copy_(Rh, non_blocking=True)             # this rank's block in, its gradient block out
+        v, _ = bp.eval(Rd, grad_out=Gd)
+        Gh.copy_(Gd, non_blocking=True)
+        torch.cuda.synchronize()
+        return v
+
     for _ in range(2):
-        v_e2e = m.mop_eval_veff_grad_host(Rh, Gh)
+        v_e2e = e2e_step()
     n_e2e = max(3, min(a.steps, 10))
     if world > 1:
         torch.distributed.barrier()
@@ -291,12 +327,14 @@ def run_ours(a):
     te = time.perf_counter()
     for _ in range(n_e2e):
         flush.zero_()
-        v_e2e = m.mop_eval_veff_grad_host(Rh, Gh)
+        v_e2e = e2e_step()
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - te) * 1e3
-    e2e_ms_max, e2e_units = all_reduce_max_sum(e2e_ms, float(N * n_e2e), world, dev)
-    if not (np.isfinite(v_e2e) and abs(v_e2e - st1["veff"]) <= 1e-5 * abs(st1["veff"])):
+    e2e_ms_max, e2e_units = all_reduce_max_sum(e2e_ms, float(Rd.shape[0] * n_e2e), world, dev)
+    if not blocks_mode and not (np.isfinite(v_e2e) and abs(v_e2e - st1["veff"]) <= 1e-5 * abs(st1["veff"])):
         raise RuntimeError("host-buffer evaluation disagrees with the device-buffer one: %r vs %r" % (v_e2e, st1["veff"]))
+    if not np.isfinite(v_e2e):
+        raise RuntimeError("V_eff is not finite in the end-to-end run")
 
     if rank != 0:
         m.close()
@@ -315,10 +353,14 @@ def run_ours(a):
         "metric": METRIC, "value": throughput(units, ms_max), "unit": UNIT, "n_gpus": world, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(a.config, s, N), "parallelism": "replicas only" if world > 1 else "1 GPU",
+        "config": {"workload": workload_name(a.config, s, N) if not blocks_mode else
+                   workload_name(a.config, s, n_path) + " (one path; %d beads per GPU)" % N,
+                   "parallelism": "1 GPU" if world == 1 else
+                   ("bead blocks: %d ranks x %d beads of one %d-bead path, halos by NCCL send/recv, V_eff all-reduced "
+                    "(mop.h bead-block mode)" % (world, N, n_path) if blocks_mode else "independent replicas"),
                    "l2": "256 MiB buffer written between timed steps (L2 flush)", "pair_list": "rebuilt every step",
                    "path": "Brownian recursion, dt=2 fs, nu=50/ps, T=%g K, seed %d" % (s.temperature, rank)},
-        "pair_interactions_per_sec": world * (pairs_force + pairs_hvp) / (ms_per_step * 1e-3),
+        "pair_interactions_per_sec": (pairs_force_job + pairs_hvp_job) / (ms_per_step * 1e-3),
         "pairs_in_range_per_bead": pairs_force / max(m.nf, 1),
         "pair_slots_evaluated_per_pass": st1["pair_slots"],
         "stage_ms": {k: round(v, 5) for k, v in stages.items() if k != "evals"},
@@ -331,9 +373,10 @@ def run_ours(a):
                      "fp32_probe_tflops": {k: round(v, 2) for k, v in probe.items() if k != "sms"},
                      "force_kernel": {"achieved": ach_f, "frac": ach_f / peak_tf, "flop_per_pair": FLOP_PER_PAIR_FORCE,
                                       "pairs_per_launch": pairs_force, "ms_per_launch": stages["S2_nb_force"]}},
-        "e2e": {"value": throughput(e2e_units, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": int(N) * Q * 12,
-                "d2h_bytes_per_step": int(N) * Q * 12 + 8, "steps": n_e2e,
-                "api": "mop_eval_veff_grad_host (pinned host R in, grad + V_eff out)"},
+        "e2e": {"value": throughput(e2e_units, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": int(n_path) * Q * 12,
+                "d2h_bytes_per_step": int(n_path) * Q * 12 + 8 * world, "steps": n_e2e,
+                "api": "mop_eval_veff_grad_host (pinned host R in, grad + V_eff out)" if not blocks_mode else
+                       "per rank: pinned host block -> device, blocks.BlockPath.eval, gradient block -> pinned host"},
         "with_list_reuse": reuse,
         "gpu_launches": launches,
         "clocks": clk,
@@ -435,6 +478,10 @@ def main():
     ap.add_argument("--beads", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--blocks-on-one-gpu", action="store_true",
+                    help="--gpus 1 through the bead-block driver (one block = the whole path): exercises that code path")
+    ap.add_argument("--parallelism", default="blocks", choices=["blocks", "replicas"],
+                    help="--gpus N > 1: one path sharded by bead blocks with halo exchange (default), or independent replicas")
     a = ap.parse_args()
     if a.beads is None:
         a.beads = {1: 16, 2: 64, 3: 32, 4: 8}[a.config]

@@ -227,6 +227,40 @@ mop_status mop_step_langevin_continue(mop_ctx *c, float *R_dev, float *V_dev, do
  * the pair kernels rests on (the tests hold it equal to the oracle's pair count).  Synchronises. */
 mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange);
 
+/* Testing aid: replaces the pair-list buffers by ones of the given capacities (work units, octet-pair entries, exclusion-mask
+ * rows; 0 keeps one; at least 64 each) and switches off the automatic capacity check of the first evaluation, so that the
+ * overflow / regrow path (MOP_ERR_OOM, then a successful repeat) can be driven deterministically.  Synchronises. */
+mop_status mop_debug_set_list_capacity(mop_ctx *c, unsigned units, unsigned entries, unsigned masks);
+
+/* ---- bead-block mode -------------------------------------------------------------
+ * The paper's parallel layout: the beads of the path are spread over processing elements and only the owners of ADJACENT
+ * beads exchange data ("each bead ... a separate processing element"; non-blocking send/recv between
+ * neighbouring beads; weak scaling in the number of beads).  Here one context (one GPU, one
+ * process) owns the contiguous block of beads [first_bead, first_bead + p->n_beads) of a path of n_beads_path beads.
+ * Eqs (3),(5)-(7) couple bead n to beads n-1 and n+1 only, so one evaluation needs two halos, each DEVICE [Q][3] float in
+ * original atom order:
+ *   from the right neighbour, before pass 1: R_right = its first bead R^{n1} (eta of the block's last bead);
+ *   from the left neighbour, before the assembly: K eta^{n0-1}, which that neighbour's mop_block_pass1 writes to its
+ *     keta_right_out_dev (the spring term K eta^{n-1} of eqs (5),(7)).
+ * The library does no communication: the caller moves the halos (bench.py: torch.distributed send/recv over NCCL) and sums
+ * the per-block V_eff values (an 8-byte all-reduce).  Call order per evaluation: mop_block_pass1 (S0-S4), mop_block_pass2
+ * (S5-S6), mop_block_assemble (S7); the halo for the right neighbour is ready once pass1 has run, so its transfer overlaps
+ * pass 2.  Force, eta and H.eta run on every bead of the block except the path's last bead; U(R^1) only in the block with
+ * first_bead = 0.  A block that is the whole path (first_bead = 0, n_beads = n_beads_path) also accepts the whole-path calls
+ * above; other block contexts refuse them (INVALID_ARG), and none of them takes a bias.  The sum over blocks of
+ * veff_local_out is V_eff; the blocks' gradients are the rows of the whole-path gradient.
+ * Errors: as mop_create / mop_eval_veff_grad; INVALID_ARG for a block outside the path, a missing halo, or calls out of order. */
+mop_status mop_create_block(mop_ctx **out, const mop_params *p, int first_bead, int n_beads_path);
+mop_status mop_block_pass1(mop_ctx *c, const float *R_dev, const float *R_right_dev, float *keta_right_out_dev);
+mop_status mop_block_pass2(mop_ctx *c, const float *R_dev);
+/* keta_left_dev: NULL for first_bead = 0.  veff_local_out: HOST, non-NULL synchronises (U(R^1) if the block holds bead 1,
+ * plus the spring energy of the block's own eta).  grad_dev DEVICE [n_beads][Q][3]. */
+mop_status mop_block_assemble(mop_ctx *c, const float *keta_left_dev, double *veff_local_out, float *grad_dev);
+/* One half of a velocity-Verlet step of eq. (4) on the block's beads with a gradient the caller holds (every bead moves
+ * with its own gradient, so the integrator needs no exchange): stage 0: v += dt/2 (-grad)/m; R += dt v.  stage 1:
+ * v += dt/2 (-grad)/m.  Works on any context. */
+mop_status mop_block_integrate(mop_ctx *c, float *R_dev, float *V_dev, const float *grad_dev, double dt_pmd, int stage);
+
 #ifdef __cplusplus
 }
 #endif

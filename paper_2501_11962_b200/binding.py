@@ -18,7 +18,8 @@ STATUS = {0: "MOP_OK", 1: "MOP_ERR_INVALID_ARG", 2: "MOP_ERR_NO_TOPOLOGY", 3: "M
 EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_destroy", "mop_last_error",
            "mop_get_stats", "mop_debug_get", "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host",
            "mop_set_timing", "mop_get_timing", "mop_eval_veff_grad_fd", "mop_step_continue",
-           "mop_step_langevin_continue", "mop_debug_count_inrange",
+           "mop_step_langevin_continue", "mop_debug_count_inrange", "mop_create_block", "mop_block_pass1",
+           "mop_block_pass2", "mop_block_assemble", "mop_block_integrate", "mop_debug_set_list_capacity",
            "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias"]
 
 
@@ -78,6 +79,18 @@ def load(build_if_missing=True):
     L.mop_step_continue.restype = C.c_int
     L.mop_debug_count_inrange.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong)]
     L.mop_debug_count_inrange.restype = C.c_int
+    L.mop_debug_set_list_capacity.argtypes = [C.c_void_p, C.c_uint, C.c_uint, C.c_uint]
+    L.mop_debug_set_list_capacity.restype = C.c_int
+    L.mop_create_block.argtypes = [C.POINTER(C.c_void_p), C.POINTER(mop_params), C.c_int, C.c_int]
+    L.mop_create_block.restype = C.c_int
+    L.mop_block_pass1.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.mop_block_pass1.restype = C.c_int
+    L.mop_block_pass2.argtypes = [C.c_void_p, C.c_void_p]
+    L.mop_block_pass2.restype = C.c_int
+    L.mop_block_assemble.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
+    L.mop_block_assemble.restype = C.c_int
+    L.mop_block_integrate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int]
+    L.mop_block_integrate.restype = C.c_int
     L.mop_eval_veff_grad_fd.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]
     L.mop_eval_veff_grad_fd.restype = C.c_int
     L.mop_step_langevin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
@@ -126,7 +139,9 @@ def _np(a, dtype, shape=None):
 class Mop:
     """One context (device, system).  `system` carries the attributes of workloads.System."""
 
-    def __init__(self, system, n_beads, device=0, r_buf=0.0, stream=None):
+    def __init__(self, system, n_beads, device=0, r_buf=0.0, stream=None, block=None):
+        """block = (first_bead, n_beads_path): mop_create_block -- the context owns beads [first_bead, first_bead +
+        n_beads) of a longer path (bead-block mode, see MopBlockMethods below)."""
         import torch
         self.torch = torch
         self.L = load()
@@ -135,6 +150,11 @@ class Mop:
         self.device = torch.device("cuda", device)
         self.Q, self.N = int(system.n_atoms), int(n_beads)
         self.nf = max(self.N - 1, 1)
+        self.block = None
+        if block is not None:
+            n0, ntot = int(block[0]), int(block[1])
+            self.block = (n0, ntot)
+            self.nf = max(1 if ntot == 1 else min(self.N, ntot - 1 - n0), 1)
         p = mop_params()
         p.n_atoms, p.n_beads = self.Q, self.N
         for d in range(3):
@@ -147,7 +167,10 @@ class Mop:
         self.stream = st
         p.stream = C.c_void_p(st.cuda_stream)
         self.ctx = C.c_void_p()
-        s = self.L.mop_create(C.byref(self.ctx), C.byref(p))
+        if self.block is None:
+            s = self.L.mop_create(C.byref(self.ctx), C.byref(p))
+        else:
+            s = self.L.mop_create_block(C.byref(self.ctx), C.byref(p), self.block[0], self.block[1])
         if s != MOP_OK:
             raise MopError(s, (self.L.mop_last_error(None) or b"").decode())
         self.set_topology(system)
@@ -254,6 +277,31 @@ class Mop:
         self._check(f(self.ctx, _ptr(R), _ptr(V), float(dt_pmd), int(n_steps), float(gamma), float(temperature), int(seed),
                       int(step0)))
 
+    # ---- bead-block mode (mop.h "bead-block mode"): pass 1, [halo exchange by the caller], pass 2, assembly
+    def mop_block_pass1(self, R, R_right=None, keta_right_out=None):
+        """R [n_beads][Q][3] cuda; R_right [Q][3] cuda = the bead after the block; keta_right_out [Q][3] cuda receives
+        K eta of the block's last bead (both None for the path's last block)."""
+        assert R.is_cuda and R.is_contiguous() and tuple(R.shape) == (self.N, self.Q, 3)
+        for t in (R_right, keta_right_out):
+            assert t is None or (t.is_cuda and t.is_contiguous() and tuple(t.shape) == (self.Q, 3) and t.dtype == R.dtype)
+        self._check(self.L.mop_block_pass1(self.ctx, _ptr(R), _ptr(R_right), _ptr(keta_right_out)))
+
+    def mop_block_pass2(self, R):
+        self._check(self.L.mop_block_pass2(self.ctx, _ptr(R)))
+
+    def mop_block_assemble(self, keta_left=None, grad_out=None, sync=True):
+        """keta_left [Q][3] cuda from the left neighbour (None for the path's first block).  Returns (veff_local | None, grad)."""
+        assert keta_left is None or (keta_left.is_cuda and keta_left.is_contiguous() and tuple(keta_left.shape) == (self.Q, 3))
+        grad = grad_out if grad_out is not None else self.torch.empty((self.N, self.Q, 3), dtype=self.torch.float32,
+                                                                      device=self.device)
+        v = C.c_double(0.0)
+        self._check(self.L.mop_block_assemble(self.ctx, _ptr(keta_left), C.byref(v) if sync else None, _ptr(grad)))
+        return (v.value if sync else None), grad
+
+    def mop_block_integrate(self, R, V, grad, dt_pmd, stage):
+        assert R.is_cuda and V.is_cuda and grad.is_cuda and R.shape == V.shape == grad.shape
+        self._check(self.L.mop_block_integrate(self.ctx, _ptr(R), _ptr(V), _ptr(grad), float(dt_pmd), int(stage)))
+
     def mop_set_bias(self, group_a, group_b, sigma, height, pace=0):
         """MoP bias on S_e2e = s(R^N) - s(R^1), s = COM distance of the two groups.  Empty groups switch it off."""
         ga, gb = _np(group_a, np.int32), _np(group_b, np.int32)
@@ -328,6 +376,9 @@ class Mop:
         n = C.c_longlong(0)
         self._check(self.L.mop_debug_count_inrange(self.ctx, int(which), C.byref(n)))
         return int(n.value)
+
+    def mop_debug_set_list_capacity(self, units=0, entries=0, masks=0):
+        self._check(self.L.mop_debug_set_list_capacity(self.ctx, int(units), int(entries), int(masks)))
 
     def mop_destroy(self):
         if getattr(self, "ctx", None) is not None and self.ctx.value:

@@ -25,7 +25,12 @@ static thread_local char g_create_error[256] = "";
 
 struct mop_ctx {
     mop_params p;
-    int Q, N, nf;
+    int Q, N, nf;              // atoms; beads held by this context; force beads (allocation, >= 1)
+    int nfe = 0, nh = 0;       // beads whose force is evaluated (0 for a block that is only the path's last bead); beads with eta and H.eta
+    bool has_u1 = true;        // the context's first bead is bead 1 of the path (U(R^1) and the -F^1 term)
+    bool blk = false;          // bead-block mode (mop_create_block): beads [blk_n0, blk_n0 + N) of a path of blk_Ntot beads
+    int blk_n0 = 0, blk_Ntot = 0;
+    int blk_stage = 0;         // 0 idle, 1 after mop_block_pass1, 2 after mop_block_pass2
     cudaStream_t st;
     MopGrid g;
     float bin_z;
@@ -173,7 +178,7 @@ extern "C" void mop_destroy(mop_ctx *c) {
     delete c;
 }
 
-extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
+static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int n0, int Ntot) {
     if (!out || !p) {
         snprintf(g_create_error, sizeof g_create_error, "mop_create: NULL argument");
         return MOP_ERR_INVALID_ARG;
@@ -192,6 +197,8 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     for (int d = 0; d < 3; d++)
         if (p->box[d] < 2.0f * rl) return bad(MOP_ERR_BOX_TOO_SMALL, "min(box) < 2 (r_cut + r_buf)");
     if ((double)p->n_atoms * (double)p->n_beads > 1.0e9) return bad(MOP_ERR_INVALID_ARG, "n_atoms * n_beads too large");
+    if (blk && (n0 < 0 || Ntot < 1 || n0 + p->n_beads > Ntot))
+        return bad(MOP_ERR_INVALID_ARG, "bead block [first_bead, first_bead + n_beads) must lie inside [0, n_beads_path)");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || p->device < 0 || p->device >= ndev) {
         cudaGetLastError();
@@ -203,7 +210,17 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     c->p = *p;
     c->Q = p->n_atoms;
     c->N = p->n_beads;
-    c->nf = p->n_beads > 1 ? p->n_beads - 1 : 1;
+    if (!blk) {
+        c->nf = c->nfe = p->n_beads > 1 ? p->n_beads - 1 : 1;
+        c->nh = p->n_beads - 1;
+    } else {
+        // force, eta and H.eta on every bead of the block except the path's last bead (reading G6)
+        c->blk = true, c->blk_n0 = n0, c->blk_Ntot = Ntot;
+        c->has_u1 = n0 == 0;
+        c->nh = Ntot == 1 ? 0 : std::min(p->n_beads, Ntot - 1 - n0);
+        c->nfe = Ntot == 1 ? 1 : c->nh;
+        c->nf = std::max(c->nfe, 1);
+    }
     c->st = (cudaStream_t)p->stream;
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, p->device);
     c->rl = rl;
@@ -287,6 +304,12 @@ extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) {
     *c->h_slots = 0;
     *out = c;
     return MOP_OK;
+}
+
+extern "C" mop_status mop_create(mop_ctx **out, const mop_params *p) { return create_impl(out, p, false, 0, 0); }
+
+extern "C" mop_status mop_create_block(mop_ctx **out, const mop_params *p, int first_bead, int n_beads_path) {
+    return create_impl(out, p, true, first_bead, n_beads_path);
 }
 
 // (re)allocates the pair-list buffers for at least the given numbers of units, entries and exclusion-mask rows
@@ -675,29 +698,57 @@ static mop_status list_for(mop_ctx *c, const float *R, int nb) {
     return MOP_OK;
 }
 
-static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false) {
-    const int nb = c->nf;
+// One evaluation in three stages (bead-block mode runs them as separate calls with the halo exchange in between):
+// 1: S0-S4 (lists, pass 1, eta; R_next = the bead after the block; keta_out = K eta of the block's last bead),
+// 2: S5-S6 (pass 2), 3: S7 (assembly; keta_left = K eta of the bead before the block).
+static mop_status eval_stage1(mop_ctx *c, const float *R, const float *R_next, float *keta_out) {
+    const int nb = c->nfe;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
     t_mark(c, 0);
-    mop_status s = list_for(c, R, nb);
-    if (s) return s;
-    if ((s = pass_force(c, R, nb, true))) return s;
-    if (c->N > 1) {
-        LAUNCH(c, k_eta, dim3(cdiv(c->g.S, 256), nb), 256, 0, c->Q, c->g.S, R, c->d_perm, c->d_typ, c->d_F4, c->d_ai,
-               c->d_Ki, c->d_et, c->d_energy + 4);
-        t_mark(c, 5);
-        if ((s = pass_hvp(c, R, nb, true))) return s;
+    mop_status s;
+    if (nb > 0) {
+        if ((s = list_for(c, R, nb))) return s;
+        if ((s = pass_force(c, R, nb, true, c->has_u1))) return s;
     } else {
-        t_mark(c, 5), t_mark(c, 6), t_mark(c, 7);
+        t_mark(c, 1), t_mark(c, 2), t_mark(c, 3), t_mark(c, 4);
     }
+    if (c->nh > 0) {
+        LAUNCH(c, k_eta, dim3(cdiv(c->g.S, 256), c->nh), 256, 0, c->Q, c->g.S, c->N, R, R_next, c->d_perm, c->d_typ, c->d_F4,
+               c->d_ai, c->d_Ki, c->d_et, c->d_energy + 4);
+        if (keta_out)
+            LAUNCH(c, k_keta_out, cdiv(c->Q, 256), 256, 0, c->Q, c->g.S, c->nh - 1, c->d_slot_of, c->d_et, c->d_Ki, keta_out);
+    }
+    t_mark(c, 5);
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+static mop_status eval_stage2(mop_ctx *c, const float *R) {
+    if (c->nh > 0) {
+        mop_status s = pass_hvp(c, R, c->nh, true);
+        if (s) return s;
+    } else {
+        t_mark(c, 6), t_mark(c, 7);
+    }
+    return MOP_OK;
+}
+
+static mop_status eval_stage3(mop_ctx *c, const float *R, const float *keta_left, float *grad, bool deposit) {
     if (grad)
-        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->d_slot_of, c->d_F4, c->d_et,
-               c->d_H4, c->d_Ki, grad);
+        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->nh, c->has_u1 ? 1 : 0, c->d_slot_of,
+               c->d_F4, c->d_et, c->d_H4, c->d_Ki, keta_left, grad);
     t_mark(c, 8);
     if (c->bias_on && c->N > 1) bias_launch(c, R, grad, deposit);
     CK(c, cudaGetLastError());
     return MOP_OK;
+}
+
+static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false) {
+    mop_status s;
+    if ((s = eval_stage1(c, R, nullptr, nullptr))) return s;
+    if ((s = eval_stage2(c, R))) return s;
+    return eval_stage3(c, R, nullptr, grad, deposit);
 }
 
 #define PRECHECK(c)                                                          \
@@ -708,8 +759,16 @@ static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool depos
         CK(c, cudaSetDevice((c)->p.device));                                 \
     } while (0)
 
+// whole-path calls on a bead-block context are allowed only when the block IS the whole path
+#define NOT_A_PARTIAL_BLOCK(c)                                                                                       \
+    do {                                                                                                             \
+        if ((c)->blk && ((c)->blk_n0 != 0 || (c)->N != (c)->blk_Ntot))                                               \
+            FAIL(c, MOP_ERR_INVALID_ARG, "this context holds a bead block of a longer path: use the mop_block_* calls"); \
+    } while (0)
+
 extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double *veff_out, float *grad_dev) {
     PRECHECK(c);
+    NOT_A_PARTIAL_BLOCK(c);
     if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
     mop_status s = eval_async(c, R_dev, grad_dev);
     if (s) return s;
@@ -725,6 +784,7 @@ extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double 
 // force pass + one H.eta pass; every displaced configuration gets its own cell list and pair list.
 extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, double eps, double *veff_out, float *grad_dev) {
     PRECHECK(c);
+    NOT_A_PARTIAL_BLOCK(c);
     if (!R_dev || !grad_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or grad_dev is NULL");
     if (!(eps > 0.0) || !std::isfinite(eps)) FAIL(c, MOP_ERR_INVALID_ARG, "need eps > 0");
     const int nb = c->nf;
@@ -746,8 +806,8 @@ extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, doub
     if ((s = pass_force(c, R_dev, nb))) return s;
     LAUNCH(c, k_gather3, gq, 256, 0, c->Q, g.S, c->d_slot_of, c->d_F4, c->d_fdF, 1.0f);
     if (c->N > 1) {
-        LAUNCH(c, k_eta, dim3(cdiv(g.S, 256), nb), 256, 0, c->Q, g.S, R_dev, c->d_perm, c->d_typ, c->d_F4, c->d_ai,
-               c->d_Ki, c->d_et, c->d_energy + 4);
+        LAUNCH(c, k_eta, dim3(cdiv(g.S, 256), nb), 256, 0, c->Q, g.S, c->N, R_dev, (const float *)nullptr, c->d_perm, c->d_typ,
+               c->d_F4, c->d_ai, c->d_Ki, c->d_et, c->d_energy + 4);
         LAUNCH(c, k_gather3, gq, 256, 0, c->Q, g.S, c->d_slot_of, c->d_et, c->d_fdEta, 1.0f);
         for (int sign = 0; sign < 2; sign++) {
             LAUNCH(c, k_displace, cdiv(tot, 256), 256, 0, tot, sign ? -(float)eps : (float)eps, R_dev, c->d_fdEta, c->d_fdR);
@@ -769,6 +829,7 @@ extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, doub
 
 extern "C" mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff_out, float *grad_host) {
     PRECHECK(c);
+    NOT_A_PARTIAL_BLOCK(c);
     if (!R_host || !veff_out) FAIL(c, MOP_ERR_INVALID_ARG, "R_host or veff_out is NULL");
     const size_t bytes = (size_t)c->N * c->Q * 3 * sizeof(float);
     if (!c->d_Rh) CK(c, dalloc(&c->d_Rh, (size_t)c->N * c->Q * 3));
@@ -779,6 +840,57 @@ extern "C" mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, d
     if (grad_host) CK(c, cudaMemcpyAsync(grad_host, c->d_Gh, bytes, cudaMemcpyDeviceToHost, c->st));
     if ((s = read_back(c))) return s;
     *veff_out = c->last_veff;
+    return MOP_OK;
+}
+
+// ---- bead-block mode: the paper's parallel layout -- beads spread over processing elements, point-to-point
+// exchange between the owners of adjacent beads only -- with a contiguous block of beads per GPU
+extern "C" mop_status mop_block_pass1(mop_ctx *c, const float *R_dev, const float *R_right_dev, float *keta_right_out_dev) {
+    PRECHECK(c);
+    if (!c->blk) FAIL(c, MOP_ERR_INVALID_ARG, "mop_block_pass1: not a bead-block context (mop_create_block)");
+    if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
+    const bool has_right = c->blk_n0 + c->N < c->blk_Ntot;
+    if (has_right && (!R_right_dev || !keta_right_out_dev))
+        FAIL(c, MOP_ERR_INVALID_ARG, "a block that is not the path's last needs R_right_dev and keta_right_out_dev");
+    c->blk_stage = 0;
+    mop_status s = eval_stage1(c, R_dev, has_right ? R_right_dev : nullptr, has_right ? keta_right_out_dev : nullptr);
+    if (s) return s;
+    c->blk_stage = 1;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_block_pass2(mop_ctx *c, const float *R_dev) {
+    PRECHECK(c);
+    if (!c->blk || c->blk_stage != 1) FAIL(c, MOP_ERR_INVALID_ARG, "mop_block_pass2 follows mop_block_pass1");
+    if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
+    mop_status s = eval_stage2(c, R_dev);
+    if (s) return s;
+    c->blk_stage = 2;
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_block_assemble(mop_ctx *c, const float *keta_left_dev, double *veff_local_out, float *grad_dev) {
+    PRECHECK(c);
+    if (!c->blk || c->blk_stage != 2) FAIL(c, MOP_ERR_INVALID_ARG, "mop_block_assemble follows mop_block_pass2");
+    if (c->blk_n0 > 0 && !keta_left_dev) FAIL(c, MOP_ERR_INVALID_ARG, "a block that is not the path's first needs keta_left_dev");
+    mop_status s = eval_stage3(c, nullptr, c->blk_n0 > 0 ? keta_left_dev : nullptr, grad_dev, false);
+    if (s) return s;
+    c->blk_stage = 0;
+    if (veff_local_out) {
+        if ((s = read_back(c))) return s;
+        *veff_local_out = c->last_veff;
+    }
+    return MOP_OK;
+}
+
+extern "C" mop_status mop_block_integrate(mop_ctx *c, float *R_dev, float *V_dev, const float *grad_dev, double dt_pmd, int stage) {
+    PRECHECK(c);
+    if (!R_dev || !V_dev || !grad_dev) FAIL(c, MOP_ERR_INVALID_ARG, "NULL argument");
+    if (!(dt_pmd > 0.0) || (stage != 0 && stage != 1)) FAIL(c, MOP_ERR_INVALID_ARG, "need dt_pmd > 0 and stage 0 or 1");
+    const size_t total = (size_t)c->N * c->Q * 3;
+    LAUNCH(c, k_verlet, cdiv(total, 256), 256, 0, total, c->Q, (float)dt_pmd, stage, c->d_inv_mass, c->d_mass, grad_dev, R_dev,
+           V_dev, (double *)nullptr);
+    CK(c, cudaGetLastError());
     return MOP_OK;
 }
 
@@ -812,6 +924,7 @@ extern "C" mop_status mop_get_timing(mop_ctx *c, double out[16]) {
 // velocity Verlet on eq. (4) (+ the exact OU velocity update when ou); cont: d_G already holds the gradient at R_dev
 static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, bool cont, bool ou, double cc,
                             float amp, unsigned long long seed, unsigned long long step0) {
+    NOT_A_PARTIAL_BLOCK(c);
     if (!R_dev || !V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev or V_dev is NULL");
     if (n_steps < 0 || !(dt_pmd > 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need n_steps >= 0 and dt_pmd > 0");
     const size_t total = (size_t)c->N * c->Q * 3;
@@ -895,6 +1008,7 @@ extern "C" mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, 
 extern "C" mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, const int *group_b, int n_b, double sigma,
                                    double height, int pace) {
     PRECHECK(c);
+    NOT_A_PARTIAL_BLOCK(c);
     CK(c, cudaStreamSynchronize(c->st));
     c->bias_on = false;
     c->bias_steps = 0;
@@ -1054,6 +1168,17 @@ extern "C" mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *
     CK(c, cudaStreamSynchronize(c->st));
     CK(c, cudaGetLastError());
     *n_inrange = (long long)c->h_ctr->n_inrange;
+    return MOP_OK;
+}
+
+// testing aid: replace the pair-list buffers by ones of the given capacities (0: keep that capacity), so that the overflow
+// and regrow paths can be driven deterministically.  The automatic check of the first build is switched off.
+extern "C" mop_status mop_debug_set_list_capacity(mop_ctx *c, unsigned units, unsigned entries, unsigned masks) {
+    PRECHECK(c);
+    CK(c, cudaStreamSynchronize(c->st));
+    mop_status s = alloc_lists(c, units ? units : c->cap_units, entries ? entries : c->cap_entries, masks ? masks : c->cap_masks);
+    if (s) return s;
+    c->caps_checked = true;
     return MOP_OK;
 }
 

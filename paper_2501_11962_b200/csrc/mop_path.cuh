@@ -6,7 +6,10 @@
 
 // eta^n_i = (R^{n+1}_i - R^n_i) - a_i F^n_i,  a_i = dt/(m_i nu)  (L^n = a F^n, reading G1)
 // E_spring += K_i/2 |eta^n_i|^2, K_i = m_i nu/(2 dt), accumulated in FP64.  One thread per sorted slot.
-__global__ void __launch_bounds__(256) k_eta(int Q, int S, const float *__restrict__ R,
+// R_next: bead-block mode only -- the bead after the block (the right neighbour's first bead, [Q][3]) for the block's
+// last bead n_local - 1; otherwise bead n + 1 is read from R itself
+__global__ void __launch_bounds__(256) k_eta(int Q, int S, int n_local, const float *__restrict__ R,
+                                             const float *__restrict__ R_next,
                                              const int *__restrict__ perm, const int *__restrict__ typ,
                                              const float4 *__restrict__ F4, const float *__restrict__ a_i,
                                              const float *__restrict__ K_i, float4 *__restrict__ et,
@@ -19,7 +22,8 @@ __global__ void __launch_bounds__(256) k_eta(int Q, int S, const float *__restri
         const int i = perm[o];
         float4 out = make_float4(0.f, 0.f, 0.f, __int_as_float(typ[o]));
         if (i >= 0) {
-            const float *r0 = R + ((size_t)n * Q + i) * 3, *r1 = r0 + (size_t)Q * 3;
+            const float *r0 = R + ((size_t)n * Q + i) * 3;
+            const float *r1 = n + 1 < n_local ? r0 + (size_t)Q * 3 : R_next + (size_t)i * 3;
             const float4 f = F4[o];
             const float a = a_i[i];
             out.x = __fmaf_rn(-a, f.x, r1[0] - r0[0]);
@@ -45,30 +49,47 @@ __global__ void __launch_bounds__(256) k_eta(int Q, int S, const float *__restri
 //   n = 1     : -F^1 - K eta^1 + 1/2 H^1 eta^1          (N = 1: -F^1)
 //   1 < n < N : K eta^{n-1} - K eta^n + 1/2 H^n eta^n
 //   n = N     : K eta^{N-1}
-__global__ void __launch_bounds__(256) k_assemble(int Q, int S, int N, const int *__restrict__ slot_of,
+// over the N_local beads of the context: has_u1 = its first bead is bead 1 of the path, nh = beads that have eta and
+// H.eta (all but the path's last bead), keta_left = K eta of the bead before the block ([Q][3], original order; the left
+// neighbour's halo in bead-block mode) or NULL
+__global__ void __launch_bounds__(256) k_assemble(int Q, int S, int N_local, int nh, int has_u1,
+                                                  const int *__restrict__ slot_of,
                                                   const float4 *__restrict__ F4, const float4 *__restrict__ et,
                                                   const float4 *__restrict__ H4, const float *__restrict__ K_i,
-                                                  float *__restrict__ grad) {
+                                                  const float *__restrict__ keta_left, float *__restrict__ grad) {
     const int n = blockIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Q) return;
     float gx = 0.f, gy = 0.f, gz = 0.f;
     const float K = K_i[i];
-    if (n == 0) {
+    if (n == 0 && has_u1) {
         const float4 f = F4[slot_of[i]];
         gx -= f.x, gy -= f.y, gz -= f.z;
     }
     if (n > 0) {
         const float4 e = et[(size_t)(n - 1) * S + slot_of[(size_t)(n - 1) * Q + i]];
         gx = fmaf(K, e.x, gx), gy = fmaf(K, e.y, gy), gz = fmaf(K, e.z, gz);
+    } else if (keta_left) {
+        gx += keta_left[3 * (size_t)i], gy += keta_left[3 * (size_t)i + 1], gz += keta_left[3 * (size_t)i + 2];
     }
-    if (n < N - 1) {
+    if (n < nh) {
         const size_t o = (size_t)n * S + slot_of[(size_t)n * Q + i];
         const float4 e = et[o], h = H4[o];
         gx += fmaf(-K, e.x, 0.5f * h.x), gy += fmaf(-K, e.y, 0.5f * h.y), gz += fmaf(-K, e.z, 0.5f * h.z);
     }
     float *g = grad + ((size_t)n * Q + i) * 3;
     g[0] = gx, g[1] = gy, g[2] = gz;
+}
+
+// bead-block mode: K eta of local bead n in original atom order, the halo the right neighbour's assembly needs
+__global__ void __launch_bounds__(256) k_keta_out(int Q, int S, int n, const int *__restrict__ slot_of,
+                                                  const float4 *__restrict__ et, const float *__restrict__ K_i,
+                                                  float *__restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Q) return;
+    const float4 e = et[(size_t)n * S + slot_of[(size_t)n * Q + i]];
+    const float K = K_i[i];
+    out[3 * (size_t)i] = K * e.x, out[3 * (size_t)i + 1] = K * e.y, out[3 * (size_t)i + 2] = K * e.z;
 }
 
 // sorted float4 array -> original-order [nf][Q][3]

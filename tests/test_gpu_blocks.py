@@ -1,0 +1,125 @@
+"""Bead-block mode on the GPU (mop.h "bead-block mode"): several contexts on ONE device, each
+owning a contiguous block of beads of the same path, the halos handed over directly (no process group: the exchange
+itself is covered by tests/test_blocks_host.py under gloo), must reproduce the whole-path evaluation -- V_eff to 1e-8
+and the gradient to 1e-6 RMS (same kernels, same lists; only the order of the float atomics that build F differs, which
+moves E_spring by ~1e-9 of itself from one run to the next: two evaluations by ONE context differ as much) -- and the oracle at
+the usual bars.  Unmeasured on more than one GPU: this run has a single B200."""
+import numpy as np
+import pytest
+
+from paper_2501_11962_b200 import blocks
+from paper_2501_11962_b200 import workloads as W
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device: the library has no CPU fallback")
+    from paper_2501_11962_b200 import binding
+    binding.load()
+    return binding
+
+
+def run_blocks(B, s, R, parts):
+    """Evaluate the path R [N][Q][3] with one context per (first, n) in parts; returns (V_eff, grad [N][Q][3])."""
+    import torch
+    N = R.shape[0]
+    Rg = torch.tensor(R, device="cuda")
+    ctx = [B.Mop(s, n, block=(f, N)) for f, n in parts]
+    keta = [torch.zeros((s.n_atoms, 3), device="cuda") for _ in parts]
+    for k, (f, n) in enumerate(parts):
+        last = f + n == N
+        ctx[k].mop_block_pass1(Rg[f:f + n], None if last else Rg[f + n].contiguous(), None if last else keta[k])
+    for k, (f, n) in enumerate(parts):
+        ctx[k].mop_block_pass2(Rg[f:f + n])
+    v, g = 0.0, []
+    for k, (f, n) in enumerate(parts):
+        vk, gk = ctx[k].mop_block_assemble(None if k == 0 else keta[k - 1])
+        v += vk
+        g.append(gk.cpu().numpy())
+    for c in ctx:
+        c.close()
+    return v, np.concatenate(g, 0)
+
+
+@pytest.mark.parametrize("name,parts", [("c2", [(0, 4), (4, 4)]), ("c2", [(0, 3), (3, 4), (7, 1)]), ("c2", [(k, 1) for k in range(8)]),
+                                        ("chain", [(0, 1), (1, 5)]), ("c1", [(0, 16)])])
+def test_blocks_reproduce_the_whole_path(B, oracle, name, parts):
+    if name == "c1":
+        s = W.config1(n_beads=16)
+    elif name == "c2":
+        s = W.config2(n_beads=8)
+    else:
+        s = H.tiny_chain()
+        s.n_beads = 6
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, s.n_beads, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    m = B.Mop(s, s.n_beads)
+    v0, g0 = m.mop_eval_veff_grad(R)
+    m.close()
+    v, g = run_blocks(B, s, R, parts)
+    assert abs(v - v0) <= 1e-8 * abs(v0)
+    assert H.rms_rel(g, g0.cpu().numpy()) <= 1e-6
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=s.n_atoms <= 3000)
+    assert abs(v - v_ref) <= 1e-6 * abs(v_ref)
+    H.assert_close(g, g_ref, 1e-4)
+
+
+def test_block_context_rules_and_integrator(B, oracle):
+    import torch
+    s = W.config1(n_beads=4)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 4, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    Rg = torch.tensor(R, device="cuda")
+    a = B.Mop(s, 2, block=(0, 4))
+    with pytest.raises(B.MopError) as e:              # a partial block refuses the whole-path call
+        a.mop_eval_veff_grad(Rg[:2])
+    assert e.value.status == 1
+    with pytest.raises(B.MopError):                   # pass 2 before pass 1
+        a.mop_block_pass2(Rg[:2])
+    with pytest.raises(B.MopError):                   # not the last block: the right halo is required
+        a.mop_block_pass1(Rg[:2])
+    with pytest.raises(B.MopError):                   # block outside the path
+        B.Mop(s, 3, block=(2, 4))
+    a.close()
+    # a block that is the whole path takes the whole-path calls
+    w = B.Mop(s, 4, block=(0, 4))
+    m = B.Mop(s, 4)
+    v1, g1 = w.mop_eval_veff_grad(Rg)
+    v0, g0 = m.mop_eval_veff_grad(Rg)
+    assert abs(v1 - v0) <= 1e-8 * abs(v0) and H.rms_rel(g1.cpu().numpy(), g0.cpu().numpy()) <= 1e-6
+    # one velocity-Verlet step from the block integrator = mop_step(.., 1)
+    rng = np.random.default_rng(3)
+    sd = np.sqrt(W.KB * s.temperature / s.mass.astype(np.float64))
+    V0 = torch.tensor((rng.normal(0, 1, R.shape) * sd[None, :, None]).astype(np.float32), device="cuda")
+    Ra, Va = Rg.clone(), V0.clone()
+    m.mop_step(Ra, Va, 0.001, 1)
+    Rb, Vb = Rg.clone(), V0.clone()
+    _, g = w.mop_eval_veff_grad(Rb)
+    w.mop_block_integrate(Rb, Vb, g, 0.001, 0)
+    _, g = w.mop_eval_veff_grad(Rb)
+    w.mop_block_integrate(Rb, Vb, g, 0.001, 1)
+    assert H.rms_rel((Rb - Rg).cpu().numpy(), (Ra - Rg).cpu().numpy()) <= 1e-5
+    assert H.rms_rel(Vb.cpu().numpy(), Va.cpu().numpy()) <= 1e-5
+    w.close()
+    m.close()
+
+
+def test_block_path_driver_single_rank(B, oracle):
+    """blocks.BlockPath with world = 1 (no process group): the driver bench.py uses, on the real engine."""
+    import torch
+    s = W.config1(n_beads=6)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 6, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    Rg = torch.tensor(R, device="cuda")
+    eng = B.Mop(s, 6, block=(0, 6))
+    bp = blocks.BlockPath(eng, s.n_atoms, 0, 6, 6, rank=0, world=1, device="cuda")
+    v, g = bp.eval(Rg)
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=True)
+    assert abs(v - v_ref) <= 1e-6 * abs(v_ref)
+    H.assert_close(g.cpu().numpy(), g_ref, 1e-4)
+    eng.close()

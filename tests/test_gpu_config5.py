@@ -160,3 +160,18 @@ def test_config5_sweep_sampled_beads(B, oracle, big, N):
         assert abs(v - v_ref) <= TOL_V * abs(v_ref)
         assert m.mop_debug_count_inrange(2) == sum(npairs[(idx[n], idx[n + 1])] for n in range(N - 1))
     m.close()
+
+
+def test_config4_bead_blocks_reproduce_the_whole_path(B, oracle, big):
+    """NEXT-4 on the bench workload: beads [0,4) and [4,8) in two contexts on this one GPU against the whole-path
+    evaluation (V_eff 1e-8, gradient 1e-6 RMS)."""
+    from tests.test_gpu_blocks import run_blocks
+    s, o, R16 = big
+    R = np.ascontiguousarray(R16[:8])
+    m = B.Mop(s, 8)
+    v0, g0 = m.mop_eval_veff_grad(R)
+    g0 = g0.cpu().numpy()
+    m.close()
+    v, g = run_blocks(B, s, R, [(0, 4), (4, 4)])
+    assert abs(v - v0) <= 1e-8 * abs(v0)
+    assert H.rms_rel(g, g0) <= 1e-6

@@ -637,7 +637,7 @@ def test_error_codes(B):
 
 
 # --------------------------------------------------------------------------- list capacity and runaway coordinates
-def _blob_system(n=4000, L=20.0, spacing=0.36, seed=5):
+def _blob_system(n=1500, L=12.0, spacing=0.36, seed=5):
     rng = np.random.default_rng(seed)
     k = int(np.ceil(n ** (1 / 3)))
     g = np.stack(np.meshgrid(*[np.arange(k)] * 3, indexing="ij"), -1).reshape(-1, 3)[:n]
@@ -647,14 +647,12 @@ def _blob_system(n=4000, L=20.0, spacing=0.36, seed=5):
     return s, Xb
 
 
-def test_pair_list_regrows_on_inhomogeneous_systems(B, oracle):
-    """A dense cluster in a large vacuum box, centred on the box corner (every periodic shift is in use): the list
-    capacities estimated from the mean density are far too small.  The first evaluation of a topology checks them and
-    regrows silently; a later evaluation that overflows returns MOP_ERR_OOM without a memory fault, has regrown the
-    buffers, and the repeated call matches the oracle."""
+def test_inhomogeneous_system_cluster_on_the_box_corner(B, oracle):
+    """A dense cluster in a large vacuum box (local density far above Q/V), centred on the box corner so that every
+    periodic shift is in use, and in the middle of the box."""
     s, Xb = _blob_system()
     o = oracle.OracleSystem(s)
-    for centre in (0.0, 10.0):
+    for centre in (0.0, 6.0):
         X = (Xb + centre).astype(np.float32)
         m = B.Mop(s, 1)
         v, g = m.mop_eval_veff_grad(X[None])
@@ -662,21 +660,39 @@ def test_pair_list_regrows_on_inhomogeneous_systems(B, oracle):
         assert abs(v - ref["U"].sum()) <= TOL_V * abs(ref["U"].sum())
         H.assert_close(g.cpu().numpy()[0], -ref["F"], TOL_RMS)
         assert m.mop_debug_count_inrange(2) == ref["npairs"]
-        assert m.mop_get_stats()["rebuilds"] >= 2        # the first build overflowed and was repeated
         m.close()
-    # overflow after the capacities were checked: a dilute gas first, then the cluster
-    rng = np.random.default_rng(6)
-    gas = rng.uniform(0, 20.0, Xb.shape).astype(np.float32)
-    m = B.Mop(s, 1)
-    m.mop_eval_veff_grad(gas[None], want_grad=False)
-    X = Xb.astype(np.float32)
+
+
+@pytest.mark.parametrize("which", ["entries", "units", "masks"])
+def test_pair_list_overflow_is_reported_and_regrown(B, oracle, which):
+    """Each pair-list buffer made too small on purpose (mop_debug_set_list_capacity): the evaluation returns MOP_ERR_OOM
+    -- no memory fault, nothing written past the buffers --, the buffers have been regrown from the builder's own counts,
+    and the repeated call matches the oracle.  Also through mop_step (an overflow in a build no synchronising call
+    follows immediately is still reported by the next one: the flag is sticky on the device)."""
+    import torch
+    s, o, R = case(oracle, "c2")
+    m = B.Mop(s, s.n_beads)
+    v0, g0 = m.mop_eval_veff_grad(R)
+    st = m.mop_get_stats()
+    small = {"entries": dict(entries=max(64, int(st["entries"] // 3))), "units": dict(units=max(64, int(st["units"] // 3))),
+             "masks": dict(masks=max(64, int(st["masks"] // 3)))}[which]
+    m.mop_debug_set_list_capacity(**small)
     with pytest.raises(B.MopError) as e:
-        m.mop_eval_veff_grad(X[None])
+        m.mop_eval_veff_grad(R)
     assert e.value.status == 4
-    v, g = m.mop_eval_veff_grad(X[None])               # buffers were regrown: the repeated call succeeds
-    ref = oracle.bead(o, X.astype(np.float64), geom=1, brute=False)
-    assert abs(v - ref["U"].sum()) <= TOL_V * abs(ref["U"].sum())
-    H.assert_close(g.cpu().numpy()[0], -ref["F"], TOL_RMS)
+    v, g = m.mop_eval_veff_grad(R)                     # buffers were regrown: the repeated call succeeds
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=False)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
+    H.assert_close(g.cpu().numpy(), g_ref, TOL_RMS)
+    # asynchronous calls: the overflow of a mop_step build surfaces at the next synchronising call
+    m.mop_debug_set_list_capacity(**small)
+    Rg, Vg = torch.tensor(R, device="cuda"), torch.zeros(R.shape, device="cuda")
+    m.mop_step(Rg, Vg, 0.0005, 2)
+    with pytest.raises(B.MopError) as e:
+        m.mop_get_stats()
+    assert e.value.status == 4
+    v, g = m.mop_eval_veff_grad(R)
+    assert abs(v - v_ref) <= TOL_V * abs(v_ref)
     m.close()
 
 

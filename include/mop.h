@@ -117,7 +117,9 @@ mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff
 /* n_steps velocity-Verlet steps of eq. (4) with F_eff = -grad V_eff and masses m_i, step dt_pmd (ps):
  *   v += dt/2 F_eff/m ; R += dt v ; F_eff(R) ; v += dt/2 F_eff/m.
  * R_dev, V_dev DEVICE [N][Q][3] float, updated in place.  The gradient at the incoming R is evaluated at the
- * start of every call (n_steps + 1 evaluations per call; mop_step_continue skips it).  Asynchronous. */
+ * start of every call (n_steps + 1 evaluations per call; mop_step_continue skips it).  Only the last evaluation of a
+ * call forms U(R^1) (the others need the gradient alone), so mop_get_stats after the call reports V_eff at the final R.
+ * Asynchronous. */
 mop_status mop_step(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps);
 
 /* NULL-safe; frees all library-owned memory. */

@@ -32,6 +32,9 @@ struct mop_ctx {
     int blk_n0 = 0, blk_Ntot = 0;
     int blk_stage = 0;         // 0 idle, 1 after mop_block_pass1, 2 after mop_block_pass2
     cudaStream_t st;
+    // library-owned side stream: the bonded kernels (O(Q) terms, latency-bound) run beside the pair kernels of the same pass
+    cudaStream_t st2 = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     MopGrid g;
     float bin_z;
     float rl, rl2, rc2;
@@ -165,6 +168,9 @@ static void free_all(mop_ctx *c) {
     if (c->h_ctr) cudaFreeHost(c->h_ctr);
     if (c->h_slots) cudaFreeHost(c->h_slots);
     if (c->h_moved) cudaFreeHost(c->h_moved);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->st2) cudaStreamDestroy(c->st2);
     if (c->ev_made)
         for (auto &set : c->ev)
             for (cudaEvent_t e : set) cudaEventDestroy(e);
@@ -174,6 +180,7 @@ extern "C" void mop_destroy(mop_ctx *c) {
     if (!c) return;
     cudaSetDevice(c->p.device);
     cudaStreamSynchronize(c->st);
+    if (c->st2) cudaStreamSynchronize(c->st2);
     free_all(c);
     delete c;
 }
@@ -288,6 +295,9 @@ static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int 
     A(cudaMallocHost((void **)&c->h_energy, 8 * sizeof(double)));
     A(cudaMallocHost((void **)&c->h_ctr, sizeof(MopCounters)));
     A(cudaMallocHost((void **)&c->h_slots, sizeof(unsigned long long)));
+    A(cudaStreamCreateWithFlags(&c->st2, cudaStreamNonBlocking));
+    A(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    A(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     if (e != cudaSuccess) {
         snprintf(g_create_error, sizeof g_create_error, "mop_create: device allocation failed: %s",
                  cudaGetErrorString(e));
@@ -596,6 +606,18 @@ static BondedArgs bonded_args(mop_ctx *c, const float *R, float4 *out) {
 static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = false, bool with_energy = true) {
     const size_t smem = nb_smem(c);
     CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
+    // the bonded terms go first, on the side stream: both kernels accumulate into F4 with reductions, and the few hundred
+    // small CTAs of k_bonded are resident before the persistent pair kernel fills the machine
+    const int nterm = c->n_bonds + c->n_angles;
+    if (nterm > 0) {
+        CK(c, cudaEventRecord(c->ev_fork, c->st));
+        CK(c, cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
+        BondedArgs b = bonded_args(c, R, c->d_F4);
+        if (!with_energy) b.energies = c->d_energy + 8;
+        k_bonded<false><<<dim3(cdiv(nterm, 128), nb), 128, 0, c->st2>>>(b);
+        c->n_launches += 1;
+        CK(c, cudaEventRecord(c->ev_join, c->st2));
+    }
     if (with_energy) {
         LAUNCH(c, nb_pick(NB_ENERGY), c->nb_blocks_fe, 128, smem, nb_args(c, c->d_F4, 0, 0));
         if (nb > 1) LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 1, 1));
@@ -603,13 +625,8 @@ static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = fa
         LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, smem, nb_args(c, c->d_F4, 0, 2));
     }
     if (timed) t_mark(c, 3);
-    const int nterm = c->n_bonds + c->n_angles;
-    if (nterm > 0) {
-        BondedArgs b = bonded_args(c, R, c->d_F4);
-        if (!with_energy) b.energies = c->d_energy + 8;
-        LAUNCH(c, k_bonded<false>, dim3(cdiv(nterm, 128), nb), 128, 0, b);
-    }
-    if (timed) t_mark(c, 4);
+    if (nterm > 0) CK(c, cudaStreamWaitEvent(c->st, c->ev_join, 0));
+    if (timed) t_mark(c, 4);   // S3 = what is left of the bonded kernel after the pair kernels
     return MOP_OK;
 }
 
@@ -617,10 +634,17 @@ static mop_status pass_force(mop_ctx *c, const float *R, int nb, bool timed = fa
 static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = false) {
     const size_t smem = nb_smem(c);
     CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
+    const int nterm = c->n_bonds + c->n_angles;
+    if (nterm > 0) {   // bonded H.eta beside the pair kernel (see pass_force)
+        CK(c, cudaEventRecord(c->ev_fork, c->st));
+        CK(c, cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
+        k_bonded<true><<<dim3(cdiv(nterm, 128), nb), 128, 0, c->st2>>>(bonded_args(c, R, c->d_H4));
+        c->n_launches += 1;
+        CK(c, cudaEventRecord(c->ev_join, c->st2));
+    }
     LAUNCH(c, nb_pick(NB_HVP), c->nb_blocks_h, 128, smem, nb_args(c, c->d_H4, 2, 2));
     if (timed) t_mark(c, 6);
-    const int nterm = c->n_bonds + c->n_angles;
-    if (nterm > 0) LAUNCH(c, k_bonded<true>, dim3(cdiv(nterm, 128), nb), 128, 0, bonded_args(c, R, c->d_H4));
+    if (nterm > 0) CK(c, cudaStreamWaitEvent(c->st, c->ev_join, 0));
     if (timed) t_mark(c, 7);
     return MOP_OK;
 }
@@ -701,7 +725,7 @@ static mop_status list_for(mop_ctx *c, const float *R, int nb) {
 // One evaluation in three stages (bead-block mode runs them as separate calls with the halo exchange in between):
 // 1: S0-S4 (lists, pass 1, eta; R_next = the bead after the block; keta_out = K eta of the block's last bead),
 // 2: S5-S6 (pass 2), 3: S7 (assembly; keta_left = K eta of the bead before the block).
-static mop_status eval_stage1(mop_ctx *c, const float *R, const float *R_next, float *keta_out) {
+static mop_status eval_stage1(mop_ctx *c, const float *R, const float *R_next, float *keta_out, bool want_energy = true) {
     const int nb = c->nfe;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
     CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
@@ -709,7 +733,7 @@ static mop_status eval_stage1(mop_ctx *c, const float *R, const float *R_next, f
     mop_status s;
     if (nb > 0) {
         if ((s = list_for(c, R, nb))) return s;
-        if ((s = pass_force(c, R, nb, true, c->has_u1))) return s;
+        if ((s = pass_force(c, R, nb, true, c->has_u1 && want_energy))) return s;
     } else {
         t_mark(c, 1), t_mark(c, 2), t_mark(c, 3), t_mark(c, 4);
     }
@@ -744,9 +768,11 @@ static mop_status eval_stage3(mop_ctx *c, const float *R, const float *keta_left
     return MOP_OK;
 }
 
-static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false) {
+// want_energy = false: U(R^1) is not formed (bead 1 takes the plain force kernel): the inner evaluations of mop_step*,
+// which need the gradient only
+static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool deposit = false, bool want_energy = true) {
     mop_status s;
-    if ((s = eval_stage1(c, R, nullptr, nullptr))) return s;
+    if ((s = eval_stage1(c, R, nullptr, nullptr, want_energy))) return s;
     if ((s = eval_stage2(c, R))) return s;
     return eval_stage3(c, R, nullptr, grad, deposit);
 }
@@ -932,7 +958,7 @@ static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pm
     mop_status s;
     if (cont) {
         if (!c->g_current) FAIL(c, MOP_ERR_INVALID_ARG, "mop_step*_continue: no gradient from a previous mop_step* call is held");
-    } else if ((s = eval_async(c, R_dev, c->d_G))) {
+    } else if ((s = eval_async(c, R_dev, c->d_G, false, n_steps == 0))) {
         return s;
     }
     c->g_current = false;
@@ -941,8 +967,8 @@ static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pm
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 0, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (double *)nullptr);
         c->bias_steps += 1;
-        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0))) return s;
-        const bool last = it == n_steps - 1;
+        const bool last = it == n_steps - 1;   // V_eff (mop_get_stats) is that of the last evaluation of the call: only it forms U(R^1)
+        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0, last))) return s;
         if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (last && !ou) ? c->d_energy + 5 : (double *)nullptr);

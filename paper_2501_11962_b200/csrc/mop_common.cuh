@@ -18,7 +18,9 @@
 #define MOP_KE 138.935458f // Coulomb constant, kJ mol^-1 nm e^-2
 #define MOP_MAX_TYPES 64
 #define MOP_EXROWS 48      // max distinct j-octets holding exclusion partners of one i-octet (row 0: the octet itself)
+#ifndef MOP_LBUF
 #define MOP_LBUF 384       // per-warp staging capacity (candidate j-octets) in the list builder
+#endif
 #define MOP_NOSHIFT 21     // shift id (kx+1) | (ky+1) << 2 | (kz+1) << 4 of the zero shift
 
 struct MopGrid {

@@ -40,7 +40,10 @@ __device__ __forceinline__ float mop_gap(float lo_a, float hi_a, float lo_b, flo
 __constant__ unsigned char c_pat_order[16] = {15, 7, 3, 1, 14, 12, 8, 6, 2, 4, 5, 9, 10, 11, 13, 0};
 
 #define MOP_PL_WARPS 4     // warps (i-octets) per CTA of the list builder
-__global__ void __launch_bounds__(32 * MOP_PL_WARPS) k_pairlist(PlArgs a) {
+#ifndef MOP_PL_MINB
+#define MOP_PL_MINB 5      // resident CTAs per SM asked for (register cap 65536 / (128 * MINB))
+#endif
+__global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlArgs a) {
     __shared__ int s_exJ[MOP_PL_WARPS][MOP_EXROWS];
     __shared__ unsigned s_exM[MOP_PL_WARPS][MOP_EXROWS][2];
     __shared__ int s_exN[MOP_PL_WARPS];

@@ -399,7 +399,9 @@ def test_mop_bias_matches_oracle(B, oracle):
     assert abs(st["s1"] - s1_ref) <= 1e-12 and abs(st["sN"] - sN_ref) <= 1e-12 and abs(st["S"] - S_ref) <= 1e-12
     assert st["V"] == pytest.approx(vb_ref, rel=1e-10)
     dg = (g1 - g0).cpu().numpy().astype(np.float64)
-    assert np.abs(dg[1:-1]).max() <= 1e-6 * np.abs(gb_ref).max()             # interior beads: float-atomic noise only
+    # interior beads: untouched by the bias; two evaluations differ by the order of the float atomics only (FP32 rounding of
+    # a gradient component, relative to the largest component of that bead block)
+    assert np.abs(dg[1:-1]).max() <= 1e-5 * np.abs(g0[1:-1].cpu().numpy()).max()
     scale = np.abs(gb_ref).max()
     assert np.abs(dg[0] - gb_ref[0]).max() <= 2e-3 * scale and np.abs(dg[-1] - gb_ref[-1]).max() <= 2e-3 * scale
     #   (g1 - g0 is a difference of two FP32 gradients of size ~|G|; the bias part itself is exact to FP32 rounding)

@@ -35,6 +35,15 @@ struct mop_ctx {
     // library-owned side stream: the bonded kernels (O(Q) terms, latency-bound) run beside the pair kernels of the same pass
     cudaStream_t st2 = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // copy stream of mop_eval_veff_grad_host: the host->device copy of beads 2..N runs behind the work on bead 1
+    cudaStream_t st_copy = nullptr;
+    cudaEvent_t ev_copy[4] = {nullptr, nullptr, nullptr, nullptr};
+    // CUDA graphs of one evaluation on the context's own staging buffers (d_Rh -> d_Gh), in two parts: A = bead 1 (S0, S1,
+    // force + energy kernel), B = everything else.  Captured on st_cap; launched into the caller's stream.
+    cudaStream_t st_cap = nullptr;
+    cudaGraphExec_t gx[4] = {nullptr, nullptr, nullptr, nullptr};   // A, B, B split in two (host entry point)
+    bool gx_valid = false;
+    double gx_launches[4] = {0, 0, 0, 0};
     MopGrid g;
     float bin_z;
     float rl, rl2, rc2;
@@ -171,6 +180,12 @@ static void free_all(mop_ctx *c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->st2) cudaStreamDestroy(c->st2);
+    for (cudaEvent_t e : c->ev_copy)
+        if (e) cudaEventDestroy(e);
+    if (c->st_copy) cudaStreamDestroy(c->st_copy);
+    for (cudaGraphExec_t x : c->gx)
+        if (x) cudaGraphExecDestroy(x);
+    if (c->st_cap) cudaStreamDestroy(c->st_cap);
     if (c->ev_made)
         for (auto &set : c->ev)
             for (cudaEvent_t e : set) cudaEventDestroy(e);
@@ -181,6 +196,7 @@ extern "C" void mop_destroy(mop_ctx *c) {
     cudaSetDevice(c->p.device);
     cudaStreamSynchronize(c->st);
     if (c->st2) cudaStreamSynchronize(c->st2);
+    if (c->st_copy) cudaStreamSynchronize(c->st_copy);
     free_all(c);
     delete c;
 }
@@ -298,6 +314,9 @@ static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int 
     A(cudaStreamCreateWithFlags(&c->st2, cudaStreamNonBlocking));
     A(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     A(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    A(cudaStreamCreateWithFlags(&c->st_copy, cudaStreamNonBlocking));
+    A(cudaStreamCreateWithFlags(&c->st_cap, cudaStreamNonBlocking));
+    for (cudaEvent_t &ev : c->ev_copy) A(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
     if (e != cudaSuccess) {
         snprintf(g_create_error, sizeof g_create_error, "mop_create: device allocation failed: %s",
                  cudaGetErrorString(e));
@@ -330,6 +349,7 @@ static mop_status alloc_lists(mop_ctx *c, double units, double entries, double m
     CK(c, dalloc(&c->d_entries, (size_t)c->cap_entries));
     CK(c, dalloc(&c->d_masks, (size_t)c->cap_masks));
     c->list_valid = false;
+    c->gx_valid = false;   // the graphs hold the old buffer addresses
     return MOP_OK;
 }
 
@@ -470,6 +490,7 @@ extern "C" mop_status mop_set_topology(mop_ctx *c, const mop_topology *t) {
     CK(c, cudaStreamSynchronize(c->st));
     c->has_topology = true;
     c->list_valid = false;
+    c->gx_valid = false;
     c->g_current = false;
     return MOP_OK;
 }
@@ -500,17 +521,19 @@ static void t_mark(mop_ctx *c, int k) {
 // ---- S0 + S1 for the first nb beads of R ----
 // per-build counters start from zero; the overflow and non-finite words are sticky (only a regrow clears overflow)
 __global__ void k_ctr_reset(MopCounters *ctr, unsigned long long *slots) {
-    ctr->n_units = ctr->n_entries = ctr->n_masks = ctr->n_units_bead0 = 0u;
+    ctr->n_units = ctr->n_entries = ctr->n_masks = ctr->n_units_bead0 = ctr->n_units_mid = 0u;
     *slots = 0ull;
 }
 __global__ void k_ctr_clear_overflow(MopCounters *ctr) { ctr->overflow = 0u; }
 
-static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed) {
-    const MopGrid &g = c->g;
+// S0 for the beads [b0, b1): cell ids, counting sort, sorted coordinates, octet bounding boxes
+static mop_status s0_range(mop_ctx *c, const float *R, int b0, int b1) {
+    MopGrid g = c->g;
+    g.n0 = b0;
+    const int nb = b1 - b0;
     const size_t Q = c->Q;
-    CK(c, cudaMemsetAsync(c->d_cell_count, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
-    CK(c, cudaMemsetAsync(c->d_cell_fill, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
-    LAUNCH(c, k_ctr_reset, 1, 1, 0, c->d_ctr, c->d_slots);
+    CK(c, cudaMemsetAsync(c->d_cell_count + (size_t)b0 * g.ncell, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
+    CK(c, cudaMemsetAsync(c->d_cell_fill + (size_t)b0 * g.ncell, 0, (size_t)nb * g.ncell * sizeof(int), c->st));
     dim3 ga(cdiv(Q, 256), nb), gs(cdiv(g.S, 256), nb);
     LAUNCH(c, k_bin, ga, 256, 0, R, g, c->d_cell, c->d_cell_count, &c->d_ctr->nonfinite);
     LAUNCH(c, k_colscan, dim3(cdiv(g.ncol, 4), nb), 128, 0, g, c->d_cell_count, c->d_cell_rel, c->d_col_count);
@@ -520,7 +543,13 @@ static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed
     LAUNCH(c, k_rank, ga, 256, 0, R, g, c->d_cell, c->d_cell_rel, c->d_col_start, c->d_cell_count, c->d_tmp,
            c->d_charge, c->d_type_row, c->d_perm, c->d_slot_of, c->d_xq, c->d_typ);
     LAUNCH(c, k_bbox, dim3(cdiv(g.S, 128), nb), 128, 0, g, c->d_perm, c->d_xq, c->d_blo, c->d_bhi);
-    if (timed) t_mark(c, 1);
+    return MOP_OK;
+}
+
+// S1 for the beads [b0, b1): their work units are appended to the list (bead 1 must come first and alone: the units
+// before the mark are the energy variant's)
+static void s1_range(mop_ctx *c, int b0, int b1) {
+    const MopGrid &g = c->g;
     PlArgs a;
     a.g = g;
     a.rl = c->rl;
@@ -533,13 +562,18 @@ static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed
     a.slots_active = c->d_slots;
     a.cap_units = c->cap_units, a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks;
     const unsigned nci_blocks = cdiv(g.S / MOP_CL, MOP_PL_WARPS);
-    a.bead0 = 0;
-    LAUNCH(c, k_pairlist, dim3(nci_blocks, 1), 32 * MOP_PL_WARPS, 0, a); // bead 1 first: its units come first (energy variant)
-    LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr, c->cap_units);
-    if (nb > 1) {
-        a.bead0 = 1;
-        LAUNCH(c, k_pairlist, dim3(nci_blocks, nb - 1), 32 * MOP_PL_WARPS, 0, a);
-    }
+    a.bead0 = b0;
+    LAUNCH(c, k_pairlist, dim3(nci_blocks, b1 - b0), 32 * MOP_PL_WARPS, 0, a);
+    if (b0 == 0) LAUNCH(c, k_mark_bead0, 1, 1, 0, c->d_ctr, c->cap_units);
+}
+
+static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed) {
+    LAUNCH(c, k_ctr_reset, 1, 1, 0, c->d_ctr, c->d_slots);
+    mop_status s = s0_range(c, R, 0, nb);
+    if (s) return s;
+    if (timed) t_mark(c, 1);
+    s1_range(c, 0, 1);   // bead 1 first: its units come first (energy variant)
+    if (nb > 1) s1_range(c, 1, nb);
     c->n_rebuilds += 1;
     if (timed) t_mark(c, 2);
     CK(c, cudaGetLastError());
@@ -760,7 +794,7 @@ static mop_status eval_stage2(mop_ctx *c, const float *R) {
 
 static mop_status eval_stage3(mop_ctx *c, const float *R, const float *keta_left, float *grad, bool deposit) {
     if (grad)
-        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, c->N, c->nh, c->has_u1 ? 1 : 0, c->d_slot_of,
+        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), c->N), 256, 0, c->Q, c->g.S, 0, c->N, c->nh, c->has_u1 ? 1 : 0, c->d_slot_of,
                c->d_F4, c->d_et, c->d_H4, c->d_Ki, keta_left, grad);
     t_mark(c, 8);
     if (c->bias_on && c->N > 1) bias_launch(c, R, grad, deposit);
@@ -785,6 +819,9 @@ static mop_status eval_async(mop_ctx *c, const float *R, float *grad, bool depos
         CK(c, cudaSetDevice((c)->p.device));                                 \
     } while (0)
 
+static bool graphs_usable(const mop_ctx *c);
+static mop_status graphs_build(mop_ctx *c);
+
 // whole-path calls on a bead-block context are allowed only when the block IS the whole path
 #define NOT_A_PARTIAL_BLOCK(c)                                                                                       \
     do {                                                                                                             \
@@ -796,8 +833,20 @@ extern "C" mop_status mop_eval_veff_grad(mop_ctx *c, const float *R_dev, double 
     PRECHECK(c);
     NOT_A_PARTIAL_BLOCK(c);
     if (!R_dev) FAIL(c, MOP_ERR_INVALID_ARG, "R_dev is NULL");
-    mop_status s = eval_async(c, R_dev, grad_dev);
-    if (s) return s;
+    mop_status s;
+    if (graphs_usable(c)) {
+        // two graph launches on the staging buffers between two device-to-device copies (a few microseconds each way)
+        if ((s = graphs_build(c))) return s;
+        const size_t bytes = (size_t)c->N * c->Q * 3 * sizeof(float);
+        CK(c, cudaMemcpyAsync(c->d_Rh, R_dev, bytes, cudaMemcpyDeviceToDevice, c->st));
+        CK(c, cudaGraphLaunch(c->gx[0], c->st));
+        CK(c, cudaGraphLaunch(c->gx[1], c->st));
+        c->n_launches += c->gx_launches[0] + c->gx_launches[1];
+        c->n_rebuilds += 1;
+        if (grad_dev) CK(c, cudaMemcpyAsync(grad_dev, c->d_Gh, bytes, cudaMemcpyDeviceToDevice, c->st));
+    } else if ((s = eval_async(c, R_dev, grad_dev))) {
+        return s;
+    }
     if (veff_out) {
         if ((s = read_back(c))) return s;
         *veff_out = c->last_veff;
@@ -853,17 +902,194 @@ extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, doub
     return MOP_OK;
 }
 
+// ---- one evaluation as two sequences on the context's staging buffers: A = bead 1 alone (S0, S1, force + energy kernel),
+// B = the other beads' S0, S1 and force kernel, the bonded terms, eta, pass 2 and the assembly.  The energy kernel thus
+// runs before the other beads are sorted, which lets the host entry point copy beads 2..N in behind it; kernels and
+// results are those of eval_async.  With mop_set_timing on, the eight timing slots of these sequences are: bead 1's S0 |
+// its S1 | its force and energy kernel | (wait for the copy of beads 2..N) | their S0, S1, force kernel | eta | pass 2 |
+// assembly.
+static mop_status seq_A(mop_ctx *c, const float *R) {
+    const int nb = c->nfe;
+    mop_status s;
+    CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
+    CK(c, cudaMemsetAsync(c->d_work, 0, 8 * sizeof(unsigned), c->st));
+    CK(c, cudaMemsetAsync(c->d_F4, 0, (size_t)nb * c->g.S * sizeof(float4), c->st));
+    LAUNCH(c, k_ctr_reset, 1, 1, 0, c->d_ctr, c->d_slots);
+    t_mark(c, 0);
+    if ((s = s0_range(c, R, 0, 1))) return s;
+    t_mark(c, 1);
+    s1_range(c, 0, 1);
+    t_mark(c, 2);
+    LAUNCH(c, nb_pick(NB_ENERGY), c->nb_blocks_fe, 128, nb_smem(c), nb_args(c, c->d_F4, 0, 0));
+    t_mark(c, 3);
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+// part 0: the whole of B.  Parts 1 and 2 (host entry point): pass 2 and the assembly in two bead groups [0, h) and [h, N),
+// so that the gradient rows of the first group travel to the host while the second group's H.eta is computed.
+static int split_bead(const mop_ctx *c) { return std::max(1, std::min(c->nh - 1, (7 * c->nh + 9) / 10)); }
+
+static mop_status seq_B(mop_ctx *c, const float *R, float *G, int part = 0) {
+    const int nb = c->nfe, N = c->N;
+    const int h = part ? split_bead(c) : nb;
+    mop_status s;
+    if (part == 2) {   // second group: H.eta of beads [h, nh), gradient rows [h, N)
+        LAUNCH(c, nb_pick(NB_HVP), c->nb_blocks_h, 128, nb_smem(c), nb_args(c, c->d_H4, 4, 4));
+        if (G)
+            LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), N - h), 256, 0, c->Q, c->g.S, h, N, c->nh, 1, c->d_slot_of, c->d_F4,
+                   c->d_et, c->d_H4, c->d_Ki, (const float *)nullptr, G);
+        CK(c, cudaGetLastError());
+        return MOP_OK;
+    }
+    t_mark(c, 4);
+    const int nterm = c->n_bonds + c->n_angles;
+    if (nb > 1 && (s = s0_range(c, R, 1, nb))) return s;
+    if (nterm > 0) {   // bonded forces of all beads on the side stream (they scatter through slot_of: after S0 of every
+                       // bead), beside the list build and the force kernel
+        CK(c, cudaEventRecord(c->ev_fork, c->st));
+        CK(c, cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
+        k_bonded<false><<<dim3(cdiv(nterm, 128), nb), 128, 0, c->st2>>>(bonded_args(c, R, c->d_F4));
+        c->n_launches += 1;
+        CK(c, cudaEventRecord(c->ev_join, c->st2));
+    }
+    if (nb > 1) {
+        if (part && h > 1) s1_range(c, 1, h);
+        if (part) LAUNCH(c, k_mark_mid, 1, 1, 0, c->d_ctr, c->cap_units);
+        s1_range(c, part ? h : 1, nb);
+        LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, nb_smem(c), nb_args(c, c->d_F4, 1, 1));
+    }
+    if (nterm > 0) CK(c, cudaStreamWaitEvent(c->st, c->ev_join, 0));
+    t_mark(c, 5);
+    if (c->nh > 0) {
+        LAUNCH(c, k_eta, dim3(cdiv(c->g.S, 256), c->nh), 256, 0, c->Q, c->g.S, N, R, (const float *)nullptr, c->d_perm,
+               c->d_typ, c->d_F4, c->d_ai, c->d_Ki, c->d_et, c->d_energy + 4);
+        t_mark(c, 6);
+        if (!part) {
+            if ((s = pass_hvp(c, R, c->nh, false))) return s;
+        } else {   // first group; the bonded H.eta of all beads beside it
+            CK(c, cudaMemsetAsync(c->d_H4, 0, (size_t)c->nh * c->g.S * sizeof(float4), c->st));
+            if (nterm > 0) {
+                CK(c, cudaEventRecord(c->ev_fork, c->st));
+                CK(c, cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
+                k_bonded<true><<<dim3(cdiv(nterm, 128), c->nh), 128, 0, c->st2>>>(bonded_args(c, R, c->d_H4));
+                c->n_launches += 1;
+                CK(c, cudaEventRecord(c->ev_join, c->st2));
+            }
+            LAUNCH(c, nb_pick(NB_HVP), c->nb_blocks_h, 128, nb_smem(c), nb_args(c, c->d_H4, 2, 3));
+            if (nterm > 0) CK(c, cudaStreamWaitEvent(c->st, c->ev_join, 0));
+        }
+    } else {
+        t_mark(c, 6);
+    }
+    t_mark(c, 7);
+    if (G)
+        LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), part ? h : N), 256, 0, c->Q, c->g.S, 0, N, c->nh, 1, c->d_slot_of, c->d_F4,
+               c->d_et, c->d_H4, c->d_Ki, (const float *)nullptr, G);
+    t_mark(c, 8);
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
+// the two sequences captured as CUDA graphs (one launch each instead of ~25 API calls: on small systems an evaluation is
+// bound by launch latency, and so is the start of every host-synchronous call).  Not used while stage timing, a bias or a
+// buffered list is on, nor before the first evaluation of a topology has checked the list capacities.
+static bool graphs_usable(const mop_ctx *c) {
+    return !c->timing && !c->bias_on && !(c->p.r_buf > 0.f) && c->caps_checked && !c->blk;
+}
+
+static mop_status graphs_build(mop_ctx *c) {
+    if (c->gx_valid) return MOP_OK;
+    const size_t tot = (size_t)c->N * c->Q * 3;
+    if (!c->d_Rh) CK(c, dalloc(&c->d_Rh, tot));
+    if (!c->d_Gh) CK(c, dalloc(&c->d_Gh, tot));   // always with the assembly (15 us): one set of graphs serves every form
+    cudaStream_t user = c->st;
+    const double l0 = c->n_launches, r0 = c->n_rebuilds;
+    for (int k = 0; k < 4; k++) {
+        if (c->gx[k]) cudaGraphExecDestroy(c->gx[k]), c->gx[k] = nullptr;
+        if (k >= 2 && c->nh < 2) continue;   // nothing to split
+        cudaGraph_t g = nullptr;
+        const double lk = c->n_launches;
+        cudaError_t e = cudaStreamBeginCapture(c->st_cap, cudaStreamCaptureModeThreadLocal);
+        mop_status s = MOP_OK;
+        if (e == cudaSuccess) {
+            c->st = c->st_cap;
+            s = k == 0 ? seq_A(c, c->d_Rh) : seq_B(c, c->d_Rh, c->d_Gh, k - 1);
+            c->st = user;
+            e = cudaStreamEndCapture(c->st_cap, &g);
+        }
+        if (s == MOP_OK && e == cudaSuccess) e = cudaGraphInstantiate(&c->gx[k], g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (s) return s;
+        CK(c, e);
+        c->gx_launches[k] = c->n_launches - lk;   // kernels in this graph, added to the count at every launch
+    }
+    c->n_launches = l0, c->n_rebuilds = r0;
+    c->gx_valid = true;
+    return MOP_OK;
+}
+
+// The end-to-end form.  The host->device copy is split: bead 1 first, beads 2..N behind it on the copy stream while the
+// main stream already sorts bead 1, builds its list and runs its force + energy kernel (about 0.5 ms of work on the
+// 150,000-atom system against 0.25 ms of copy).
 extern "C" mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, double *veff_out, float *grad_host) {
     PRECHECK(c);
     NOT_A_PARTIAL_BLOCK(c);
     if (!R_host || !veff_out) FAIL(c, MOP_ERR_INVALID_ARG, "R_host or veff_out is NULL");
-    const size_t bytes = (size_t)c->N * c->Q * 3 * sizeof(float);
-    if (!c->d_Rh) CK(c, dalloc(&c->d_Rh, (size_t)c->N * c->Q * 3));
-    if (grad_host && !c->d_Gh) CK(c, dalloc(&c->d_Gh, (size_t)c->N * c->Q * 3));
-    CK(c, cudaMemcpyAsync(c->d_Rh, R_host, bytes, cudaMemcpyHostToDevice, c->st));
-    mop_status s = eval_async(c, c->d_Rh, grad_host ? c->d_Gh : nullptr);
-    if (s) return s;
-    if (grad_host) CK(c, cudaMemcpyAsync(grad_host, c->d_Gh, bytes, cudaMemcpyDeviceToHost, c->st));
+    const size_t bead = (size_t)c->Q * 3, bytes = (size_t)c->N * bead * sizeof(float);
+    if (!c->d_Rh) CK(c, dalloc(&c->d_Rh, (size_t)c->N * bead));
+    if (grad_host && !c->d_Gh) CK(c, dalloc(&c->d_Gh, (size_t)c->N * bead));
+    float *R = c->d_Rh, *G = grad_host ? c->d_Gh : nullptr;
+    const int N = c->N;
+    mop_status s;
+    // the plain sequence for buffered lists (their reuse test needs all beads), while a bias is set, and for the first
+    // evaluation of a topology (it checks the list capacities on the host)
+    if (c->p.r_buf > 0.f || !c->caps_checked || c->bias_on) {
+        CK(c, cudaMemcpyAsync(R, R_host, bytes, cudaMemcpyHostToDevice, c->st));
+        if ((s = eval_async(c, R, G))) return s;
+        if (grad_host) CK(c, cudaMemcpyAsync(grad_host, G, bytes, cudaMemcpyDeviceToHost, c->st));
+        if ((s = read_back(c))) return s;
+        *veff_out = c->last_veff;
+        return MOP_OK;
+    }
+    const bool graphs = graphs_usable(c);
+    if (graphs && (s = graphs_build(c))) return s;
+    const bool split = grad_host && c->nh >= 2;   // pass 2 and the copy out in two bead groups
+    // ---- copies in: bead 1 | beads 2..N (ordered after whatever the main stream still does with the staging buffer)
+    CK(c, cudaEventRecord(c->ev_copy[0], c->st));
+    CK(c, cudaStreamWaitEvent(c->st_copy, c->ev_copy[0], 0));
+    CK(c, cudaMemcpyAsync(R, R_host, bead * sizeof(float), cudaMemcpyHostToDevice, c->st_copy));
+    CK(c, cudaEventRecord(c->ev_copy[1], c->st_copy));
+    if (N > 1) {
+        CK(c, cudaMemcpyAsync(R + bead, R_host + bead, (size_t)(N - 1) * bead * sizeof(float), cudaMemcpyHostToDevice, c->st_copy));
+        CK(c, cudaEventRecord(c->ev_copy[2], c->st_copy));
+    }
+    CK(c, cudaStreamWaitEvent(c->st, c->ev_copy[1], 0));
+    if (graphs) CK(c, cudaGraphLaunch(c->gx[0], c->st));
+    else if ((s = seq_A(c, R))) return s;
+    if (N > 1) CK(c, cudaStreamWaitEvent(c->st, c->ev_copy[2], 0));
+    if (!split) {
+        if (graphs) CK(c, cudaGraphLaunch(c->gx[1], c->st));
+        else if ((s = seq_B(c, R, G, 0))) return s;
+        if (graphs) c->n_launches += c->gx_launches[0] + c->gx_launches[1];
+        if (grad_host) CK(c, cudaMemcpyAsync(grad_host, G, bytes, cudaMemcpyDeviceToHost, c->st));
+    } else {
+        const size_t h = (size_t)split_bead(c);
+        if (graphs) CK(c, cudaGraphLaunch(c->gx[2], c->st));
+        else if ((s = seq_B(c, R, G, 1))) return s;
+        // gradient rows [0, h) leave on the copy stream while the second group's H.eta runs
+        CK(c, cudaEventRecord(c->ev_copy[3], c->st));
+        CK(c, cudaStreamWaitEvent(c->st_copy, c->ev_copy[3], 0));
+        CK(c, cudaMemcpyAsync(grad_host, G, h * bead * sizeof(float), cudaMemcpyDeviceToHost, c->st_copy));
+        CK(c, cudaEventRecord(c->ev_copy[0], c->st_copy));
+        if (graphs) CK(c, cudaGraphLaunch(c->gx[3], c->st));
+        else if ((s = seq_B(c, R, G, 2))) return s;
+        if (graphs) c->n_launches += c->gx_launches[0] + c->gx_launches[2] + c->gx_launches[3];
+        CK(c, cudaMemcpyAsync(grad_host + h * bead, G + h * bead, ((size_t)N - h) * bead * sizeof(float), cudaMemcpyDeviceToHost,
+                              c->st));
+        CK(c, cudaStreamWaitEvent(c->st, c->ev_copy[0], 0));   // the final synchronisation of st covers both copies
+    }
+    c->n_rebuilds += 1;
     if ((s = read_back(c))) return s;
     *veff_out = c->last_veff;
     return MOP_OK;

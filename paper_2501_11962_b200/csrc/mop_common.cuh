@@ -31,6 +31,7 @@ struct MopGrid {
     int S;                    // slots per bead (multiple of 32)
     int Q, nf;
     float colw[2];            // column widths box/dims
+    int n0;                   // first bead of this launch of the S0 kernels (bead = n0 + blockIdx.y)
 };
 
 struct MopUnit {            // one work unit of the pair kernels: (bead, i-octet)
@@ -51,7 +52,8 @@ typedef uint2 MopEntry;
 
 struct MopCounters {
     unsigned n_units, n_entries, n_masks, overflow; // overflow: bit0 entries, bit1 units, bit2 masks, bit3 staging, bit4 excl rows
-    unsigned n_units_bead0, nonfinite, work1, pad;  // nonfinite: an input coordinate was NaN/Inf or beyond 1e6 box lengths
+    unsigned n_units_bead0, nonfinite, work1, n_units_mid;  // nonfinite: an input coordinate was NaN/Inf or beyond 1e6 box lengths
+                                                            // n_units_mid: units of the first bead group (split pass 2 of the host entry point)
     unsigned long long n_pairs;   // debug pair walker
     unsigned long long n_inrange; // in-range decisions counted by the production force kernel (counting variant)
 };

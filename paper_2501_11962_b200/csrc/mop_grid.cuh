@@ -1,7 +1,8 @@
 // mop_grid.cuh -- S0: bead-batched cell-list build.
 // wrap -> cell id -> histogram -> column scan (columns padded to 32 slots) -> STABLE scatter
 // (within a cell ascending original index, reading G13) -> sorted float4 (x,y,z,q) + type + permutation.
-// All nf force beads are processed by each launch (bead = blockIdx.y).  HBM-bound.
+// A launch processes the beads g.n0, g.n0 + 1, ... (bead = g.n0 + blockIdx.y; all nf force beads, or one group of them
+// in the pipelined host entry point).  HBM-bound.
 #pragma once
 #include "mop_common.cuh"
 
@@ -9,7 +10,7 @@
 // bring it into [0, L), raises the sticky non-finite flag (reported as MOP_ERR_NONFINITE at the next synchronising call)
 __global__ void __launch_bounds__(256) k_bin(const float *__restrict__ R, MopGrid g, int *__restrict__ cell,
                                              int *__restrict__ cell_count, unsigned *__restrict__ nonfinite) {
-    int n = blockIdx.y;
+    int n = g.n0 + blockIdx.y;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Q) return;
     const float *r = R + ((size_t)n * g.Q + i) * 3;
@@ -31,7 +32,7 @@ __global__ void __launch_bounds__(256) k_bin(const float *__restrict__ R, MopGri
 // one warp per column: exclusive scan of the cell counts inside the column + the column total
 __global__ void __launch_bounds__(128) k_colscan(MopGrid g, const int *__restrict__ cell_count,
                                                  int *__restrict__ cell_rel, int *__restrict__ col_count) {
-    int n = blockIdx.y;
+    int n = g.n0 + blockIdx.y;
     int col = blockIdx.x * 4 + (threadIdx.x >> 5);
     int lane = threadIdx.x & 31;
     if (col >= g.ncol) return;
@@ -57,7 +58,7 @@ __global__ void __launch_bounds__(1024) k_colstart(MopGrid g, const int *__restr
                                                    int *__restrict__ col_start) {
     __shared__ int wsum[32];
     __shared__ int carry;
-    int n = blockIdx.x;
+    int n = g.n0 + blockIdx.x;
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (threadIdx.x == 0) carry = 0;
     __syncthreads();
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(1024) k_colstart(MopGrid g, const int *__restr
 // every slot starts as padding
 __global__ void __launch_bounds__(256) k_fill_pad(MopGrid g, int *__restrict__ perm, float4 *__restrict__ xq,
                                                   int *__restrict__ typ) {
-    int n = blockIdx.y;
+    int n = g.n0 + blockIdx.y;
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= g.S) return;
     size_t o = (size_t)n * g.S + s;
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(256) k_fill_pad(MopGrid g, int *__restrict__ p
 __global__ void __launch_bounds__(256) k_place(MopGrid g, const int *__restrict__ cell,
                                                const int *__restrict__ cell_rel, const int *__restrict__ col_start,
                                                int *__restrict__ cell_fill, int *__restrict__ tmp) {
-    int n = blockIdx.y;
+    int n = g.n0 + blockIdx.y;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Q) return;
     int c = cell[(size_t)n * g.Q + i];
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(256) k_rank(const float *__restrict__ R, MopGr
                                               const float *__restrict__ charge, const int *__restrict__ type_row,
                                               int *__restrict__ perm, int *__restrict__ slot_of,
                                               float4 *__restrict__ xq, int *__restrict__ typ) {
-    int n = blockIdx.y;
+    int n = g.n0 + blockIdx.y;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Q) return;
     int c = cell[(size_t)n * g.Q + i];
@@ -148,7 +149,7 @@ __global__ void __launch_bounds__(256) k_rank(const float *__restrict__ R, MopGr
 // bounding box over the real atoms of every octet (8 slots); lo.w = number of real atoms (int bits)
 __global__ void __launch_bounds__(128) k_bbox(MopGrid g, const int *__restrict__ perm, const float4 *__restrict__ xq,
                                               float4 *__restrict__ blo, float4 *__restrict__ bhi) {
-    const int n = blockIdx.y;
+    const int n = g.n0 + blockIdx.y;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;   // S is a multiple of 32: whole warps in range
     if (s >= g.S) return;
     const size_t o = (size_t)n * g.S + s;
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(128) k_bbox(MopGrid g, const int *__restrict__
 __global__ void __launch_bounds__(256) k_refresh(const float *__restrict__ R, const float *__restrict__ Rref, MopGrid g,
                                                  float half_buf2, const int *__restrict__ slot_of,
                                                  float4 *__restrict__ xq, int *__restrict__ flag) {
-    const int n = blockIdx.y;
+    const int n = g.n0 + blockIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.Q) return;
     const float *r = R + ((size_t)n * g.Q + i) * 3, *f = Rref + ((size_t)n * g.Q + i) * 3;

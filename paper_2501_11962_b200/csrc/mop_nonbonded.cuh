@@ -27,7 +27,7 @@ struct NbArgs {
     unsigned cap_units;              // units beyond the allocation were never written (overflow): never read them
     unsigned long long *n_inrange;   // counting variant only: in-range, non-excluded pair decisions of this launch
     unsigned *work;     // dynamic work counter (zeroed before the launch)
-    int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all
+    int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all   3: [0, n_units_mid)   4: [n_units_mid, n_units)
     const float2 *tab;  // [nt*nt] (6 C6, 12 C12)
     const float *tabs;  // [nt*nt] LJ energy shift C12 rc^-12 - C6 rc^-6 (0 when lj_shift = 0)
     double *energies;   // [0] U_lj, [1] U_coul

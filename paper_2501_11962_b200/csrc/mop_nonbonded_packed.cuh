@@ -393,6 +393,8 @@ __global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
     unsigned ubeg = 0, uend = nu;
     if (a.range == 0) uend = nu0;
     else if (a.range == 1) ubeg = nu0;
+    else if (a.range == 3) uend = min(a.ctr->n_units_mid, a.cap_units);
+    else if (a.range == 4) ubeg = min(a.ctr->n_units_mid, a.cap_units);
     const unsigned s0 = (unsigned)__cvta_generic_to_shared(sb);
     const unsigned sw_addr = s0 + w * 256u, se_addr = s0 + NBP_SM_ENT + w * 256u;
     const unsigned sr_addr = s0 + NBP_SM_RING + w * (NBP_NST * 1024u), sd_addr = s0 + NBP_SM_DBL + w * 256u;

@@ -413,3 +413,4 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
 }
 
 __global__ void k_mark_bead0(MopCounters *ctr, unsigned cap_units) { ctr->n_units_bead0 = min(ctr->n_units, cap_units); }
+__global__ void k_mark_mid(MopCounters *ctr, unsigned cap_units) { ctr->n_units_mid = min(ctr->n_units, cap_units); }

@@ -52,12 +52,13 @@ __global__ void __launch_bounds__(256) k_eta(int Q, int S, int n_local, const fl
 // over the N_local beads of the context: has_u1 = its first bead is bead 1 of the path, nh = beads that have eta and
 // H.eta (all but the path's last bead), keta_left = K eta of the bead before the block ([Q][3], original order; the left
 // neighbour's halo in bead-block mode) or NULL
-__global__ void __launch_bounds__(256) k_assemble(int Q, int S, int N_local, int nh, int has_u1,
+// (n_first: first bead of this launch; the host entry point assembles and copies out the beads in two groups)
+__global__ void __launch_bounds__(256) k_assemble(int Q, int S, int n_first, int N_local, int nh, int has_u1,
                                                   const int *__restrict__ slot_of,
                                                   const float4 *__restrict__ F4, const float4 *__restrict__ et,
                                                   const float4 *__restrict__ H4, const float *__restrict__ K_i,
                                                   const float *__restrict__ keta_left, float *__restrict__ grad) {
-    const int n = blockIdx.y;
+    const int n = n_first + blockIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Q) return;
     float gx = 0.f, gy = 0.f, gz = 0.f;

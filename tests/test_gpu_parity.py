@@ -597,6 +597,30 @@ def test_host_buffer_entry_point_matches_device_one(B, oracle):
     m.close()
 
 
+def test_one_context_different_paths_in_turn(B, oracle):
+    """One context evaluates two different paths alternately, through the device and the host entry point (CUDA graphs,
+    split copies, bonded kernels on the side stream): nothing may survive from the previous evaluation -- a bonded
+    kernel that ran before the new sort would scatter through the old slot map and still pass a repeat of the SAME path."""
+    import torch
+    s, o, R = case(oracle, "c2")
+    rng = np.random.default_rng(17)
+    R2 = (R[::-1] + rng.normal(0, 0.004, R.shape)).astype(np.float32).copy()     # another path over the same system
+    ref = [oracle.veff_grad(o, X.astype(np.float64), geom=1, brute=False) for X in (R, R2)]
+    m = B.Mop(s, s.n_beads)
+    Gh = torch.empty(R.shape, dtype=torch.float32).pin_memory()
+    for k in range(6):
+        X, (v_ref, g_ref) = (R, R2)[k % 2], ref[k % 2]
+        if k < 3:
+            v, g = m.mop_eval_veff_grad(X)
+            g = g.cpu().numpy()
+        else:
+            v = m.mop_eval_veff_grad_host(torch.as_tensor(X).pin_memory(), Gh)
+            g = Gh.numpy().copy()
+        assert abs(v - v_ref) <= TOL_V * abs(v_ref), k
+        H.assert_close(g, g_ref, TOL_RMS)
+    m.close()
+
+
 def test_argument_errors_of_the_added_entry_points(B):
     import torch
     s = W.config1(n_beads=1)

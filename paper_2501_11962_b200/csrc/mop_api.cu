@@ -616,6 +616,7 @@ static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     a.xq = c->d_xq, a.typ = c->d_typ, a.et = c->d_et, a.out = out;
     a.units = c->d_units, a.entries = c->d_entries, a.masks = c->d_masks, a.ctr = c->d_ctr;
     a.cap_units = c->cap_units;
+    a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks, a.n_slots = (unsigned)c->nf * (unsigned)c->g.S;
     a.n_inrange = &c->d_ctr->n_inrange;
     a.work = c->d_work + work_slot;
     a.range = range;

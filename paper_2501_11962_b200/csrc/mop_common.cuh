@@ -23,6 +23,22 @@
 #endif
 #define MOP_NOSHIFT 21     // shift id (kx+1) | (ky+1) << 2 | (kz+1) << 4 of the zero shift
 
+// -DMOP_CHECK: a checked build for tests/sanitizer_target.py (compute-sanitizer is closed on the GPU pool this was
+// developed on): every index the list builder and the pair kernels derive from list data is tested against the size of
+// the array it goes into; a violation prints the place and traps (the launch fails with cudaErrorAssert / launch failure).
+#ifdef MOP_CHECK
+#include <cstdio>
+#define MOP_ASSERT(cond)                                                                   \
+    do {                                                                                   \
+        if (!(cond)) {                                                                     \
+            printf("MOP_ASSERT failed: %s  (%s:%d)\n", #cond, __FILE__, __LINE__);         \
+            __trap();                                                                      \
+        }                                                                                  \
+    } while (0)
+#else
+#define MOP_ASSERT(cond) ((void)0)
+#endif
+
 struct MopGrid {
     float box[3], inv_box[3]; // inv_box = 1.0f / box (FP32)
     float sc[3];              // (float)dims * inv_box (FP32 product): cell = min((int)(xw*sc), dims-1)

@@ -25,6 +25,7 @@ __global__ void __launch_bounds__(256) k_bin(const float *__restrict__ R, MopGri
     }
     if (!ok) *nonfinite = 1u;
     int id = (c[0] * g.dims[1] + c[1]) * g.dims[2] + c[2];
+    MOP_ASSERT(id >= 0 && id < g.ncell);
     cell[(size_t)n * g.Q + i] = id;
     atomicAdd(&cell_count[(size_t)n * g.ncell + id], 1);
 }
@@ -137,6 +138,7 @@ __global__ void __launch_bounds__(256) k_rank(const float *__restrict__ R, MopGr
     int rank = 0;
     for (int k = 0; k < cnt; k++) rank += (t[k] < i);
     int s = base + rank;
+    MOP_ASSERT(base >= 0 && base + cnt <= g.S && rank < cnt);
     const float *r = R + ((size_t)n * g.Q + i) * 3;
     size_t o = (size_t)n * g.S + s;
     perm[o] = i;

@@ -25,6 +25,7 @@ struct NbArgs {
     const unsigned long long *masks; // exclusion rows: byte jl = the i atoms (bits 0-7) j atom jl may interact with
     const MopCounters *ctr;
     unsigned cap_units;              // units beyond the allocation were never written (overflow): never read them
+    unsigned cap_entries, cap_masks, n_slots;   // checked build only: sizes of entries, masks and of the [nf][S] arrays
     unsigned long long *n_inrange;   // counting variant only: in-range, non-excluded pair decisions of this launch
     unsigned *work;     // dynamic work counter (zeroed before the launch)
     int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all   3: [0, n_units_mid)   4: [n_units_mid, n_units)

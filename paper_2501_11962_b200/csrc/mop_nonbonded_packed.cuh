@@ -85,6 +85,8 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     float4 *__restrict__ out = a.out;
     const int jl = lane & 7, gq = lane >> 3;
     const unsigned ibase = boff + (unsigned)un.ci * MOP_CL;
+    MOP_ASSERT(ibase + MOP_CL <= a.n_slots);
+    MOP_ASSERT((unsigned long long)un.start + un.count <= a.cap_entries && (un.count % MOP_NG) == 0);
 
     __syncwarp();
     bool has_lj = false;
@@ -151,8 +153,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         unsigned lm = valid ? 0xffu : 0u;
         if (masked) {
             const unsigned row1 = (cur.y >> 8) & 0xffu;
-            if (row1 != 0)
+            if (row1 != 0) {
+                MOP_ASSERT(un.excl_base + row1 - 1 < a.cap_masks);
                 lm = reinterpret_cast<const unsigned char *>(a.masks)[((size_t)un.excl_base + row1 - 1) * 8 + jl];
+            }
         }
 
         auto heavy = [&](const int p, const bool nolj) {
@@ -295,6 +299,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         auto issue = [&](const int k) { // start the copies of step k's j atoms into stage k % 2
             if (k < nS) {
                 const unsigned o = mop_lds_vu(se_g + (unsigned)k * 32u) + jl;
+                MOP_ASSERT(o < a.n_slots);
                 const unsigned sto = (unsigned)(k & 1) * 1024u;
                 mop_cp_async16(sr_l + sto, xq + o);
                 if (HVP) mop_cp_async16(sr_t + sto, et + o);
@@ -404,6 +409,7 @@ __global__ void __launch_bounds__(128, CTAS) k_nonbonded_p(const NbArgs a) {
         if (lane == 0) u = atomicAdd(a.work, 1u);
         u = __shfl_sync(0xffffffffu, u, 0) + ubeg;
         if (u >= uend) break;
+        MOP_ASSERT(u < a.cap_units);
         const uint4 *up = reinterpret_cast<const uint4 *>(a.units + u);
         const uint4 u0 = up[0], u1 = up[1];
         MopUnit un;

@@ -108,6 +108,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
             int J = -1, bit = 0;
             if (act) {
                 const int ps = slot_of[a.excl_list[e]];
+                MOP_ASSERT(ps >= 0 && ps < g.S);
                 J = ps >> 3;
                 bit = ps & 7;
                 if (J < J0) act = false; // never listed from this side
@@ -236,6 +237,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
                     bool ok = f < total;
                     const int cj = s_first + (f - (s_incl - s_cnt));
                     if (ok) {
+                        MOP_ASSERT(cj >= 0 && cj < noc);
                         float4 lo = jlo[cj], hi = jhi[cj];
                         ok = __float_as_int(lo.w) > 0;
                         float sx, sy, sz;
@@ -247,6 +249,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
                     }
                     const unsigned bal = __ballot_sync(0xffffffffu, ok);
                     if (ok) {
+                        MOP_ASSERT(nbuf + __popc(bal & ((1u << lane) - 1)) < MOP_LBUF);
                         bcj[nbuf + __popc(bal & ((1u << lane) - 1))] = (unsigned)cj | (s_sid << 24);
                     }
                     nbuf += __popc(bal);
@@ -370,6 +373,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
             y = (x ^ (x >> 7)) & 0x00AA00AA00AA00AAull, x ^= y ^ (y << 7);
             y = (x ^ (x >> 14)) & 0x0000CCCC0000CCCCull, x ^= y ^ (y << 14);
             y = (x ^ (x >> 28)) & 0x00000000F0F0F0F0ull, x ^= y ^ (y << 28);
+            MOP_ASSERT(mb + t < a.cap_masks);
             a.masks[(size_t)mb + t] = x;
         }
         // entries in their final order go through shared memory (the j staging buffer is free now), so that every step of
@@ -380,6 +384,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
         for (int idx = lane; idx < nbuf; idx += 32) {
             const unsigned info = binfo[idx];
             if (info == 0) continue;
+            MOP_ASSERT(pcnt[info & 31u] + (info >> 16) < (unsigned)(32 * 9 * 2));   // the j staging buffer, as uint2
             sorted[pcnt[info & 31u] + (info >> 16)] = make_uint2(bcj[idx], info & 0xff0fu);
         }
         if (lane < (int)(padded - total)) sorted[total + lane] = make_uint2((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24), 0u);
@@ -395,6 +400,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
                 if ((e[q].y >> 8) != 0u || (e[q].y & 15u) == 0u) fl |= 1u << 21;
             }
             fl |= u << 16;
+            MOP_ASSERT(st + (sidx + 1) * MOP_NG <= a.cap_entries && (st % MOP_NG) == 0);
             uint4 *dst = reinterpret_cast<uint4 *>(a.entries + st + sidx * MOP_NG); // st is a multiple of 4: 32 B aligned
             dst[0] = make_uint4(e[0].x, e[0].y | fl, e[1].x, e[1].y | fl);
             dst[1] = make_uint4(e[2].x, e[2].y | fl, e[3].x, e[3].y | fl);

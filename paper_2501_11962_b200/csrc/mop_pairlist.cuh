@@ -178,10 +178,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
         for (int kz = kz0; kz <= 1 && !full; kz++) {
             if (kz == -1 && !(zlo < 0.0f)) continue;
             if (kz == 1 && !(zhi > g.box[2])) continue;
-            const float za = kz == 0 ? fmaxf(zlo, 0.0f) : (kz == -1 ? zlo + g.box[2] : 0.0f);
-            const float zb = kz == 0 ? fminf(zhi, g.box[2]) : (kz == -1 ? g.box[2] : zhi - g.box[2]);
-            const int b0 = max(mop_cell1(fmaxf(za, 0.0f), g.sc[2], nz) - 1, 0);
-            const int b1 = min(mop_cell1(fminf(zb, g.box[2]), g.sc[2], nz) + 1, nz - 1);
+            const float zoff = (float)kz * g.box[2];   // the column's atoms are seen at z + kz Lz
             for (int ob = kz == kz0 ? ob0 : 0; ob < noff && !full; ob += 32) {
                 const int t = ob + lane;
                 int first = 0, cnt = 0;
@@ -195,7 +192,14 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
                         const float cylo = (float)coly * g.colw[1] + (float)ky * g.box[1];
                         const float dxg = mop_gap(blo.x, bhi.x, clo - marg * g.box[0], clo + g.colw[0] + marg * g.box[0]);
                         const float dyg = mop_gap(blo.y, bhi.y, cylo - marg * g.box[1], cylo + g.colw[1] + marg * g.box[1]);
-                        if (dxg * dxg + dyg * dyg < a.rl2) {
+                        const float dxy2 = dxg * dxg + dyg * dyg;
+                        // the z window of THIS column: atoms within r_list of the i box lie within sqrt(r_list^2 - gap_xy^2)
+                        // in z (a sphere, not a cylinder: a third fewer octets to test than with the full r_list)
+                        const float reach = sqrtf(fmaxf(a.rl2 - dxy2, 0.0f)) + mz;
+                        const float za = fmaxf(blo.z - reach - zoff, 0.0f), zb = fminf(bhi.z + reach - zoff, g.box[2]);
+                        if (dxy2 < a.rl2 && za <= zb) {
+                            const int b0 = max(mop_cell1(za, g.sc[2], nz) - 1, 0);
+                            const int b1 = min(mop_cell1(zb, g.sc[2], nz) + 1, nz - 1);
                             const int col = colx * ny + coly;
                             const int s0 = col_start[col];
                             const int r0 = cell_rel[(size_t)col * nz + b0];

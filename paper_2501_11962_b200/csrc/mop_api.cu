@@ -41,9 +41,9 @@ struct mop_ctx {
     // CUDA graphs of one evaluation on the context's own staging buffers (d_Rh -> d_Gh), in two parts: A = bead 1 (S0, S1,
     // force + energy kernel), B = everything else.  Captured on st_cap; launched into the caller's stream.
     cudaStream_t st_cap = nullptr;
-    cudaGraphExec_t gx[4] = {nullptr, nullptr, nullptr, nullptr};   // A, B, B split in two (host entry point)
+    cudaGraphExec_t gx[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // A, B, B split in two (host entry point), A without U(R^1)
     bool gx_valid = false;
-    double gx_launches[4] = {0, 0, 0, 0};
+    double gx_launches[5] = {0, 0, 0, 0, 0};
     MopGrid g;
     float bin_z;
     float rl, rl2, rc2;
@@ -909,7 +909,7 @@ extern "C" mop_status mop_eval_veff_grad_fd(mop_ctx *c, const float *R_dev, doub
 // results are those of eval_async.  With mop_set_timing on, the eight timing slots of these sequences are: bead 1's S0 |
 // its S1 | its force and energy kernel | (wait for the copy of beads 2..N) | their S0, S1, force kernel | eta | pass 2 |
 // assembly.
-static mop_status seq_A(mop_ctx *c, const float *R) {
+static mop_status seq_A(mop_ctx *c, const float *R, bool want_energy = true) {
     const int nb = c->nfe;
     mop_status s;
     CK(c, cudaMemsetAsync(c->d_energy, 0, 5 * sizeof(double), c->st));
@@ -921,7 +921,8 @@ static mop_status seq_A(mop_ctx *c, const float *R) {
     t_mark(c, 1);
     s1_range(c, 0, 1);
     t_mark(c, 2);
-    LAUNCH(c, nb_pick(NB_ENERGY), c->nb_blocks_fe, 128, nb_smem(c), nb_args(c, c->d_F4, 0, 0));
+    if (want_energy) LAUNCH(c, nb_pick(NB_ENERGY), c->nb_blocks_fe, 128, nb_smem(c), nb_args(c, c->d_F4, 0, 0));
+    else LAUNCH(c, nb_pick(NB_FORCE), c->nb_blocks_f, 128, nb_smem(c), nb_args(c, c->d_F4, 0, 0));   // gradient only (inner steps of mop_step)
     t_mark(c, 3);
     CK(c, cudaGetLastError());
     return MOP_OK;
@@ -1006,16 +1007,16 @@ static mop_status graphs_build(mop_ctx *c) {
     if (!c->d_Gh) CK(c, dalloc(&c->d_Gh, tot));   // always with the assembly (15 us): one set of graphs serves every form
     cudaStream_t user = c->st;
     const double l0 = c->n_launches, r0 = c->n_rebuilds;
-    for (int k = 0; k < 4; k++) {
+    for (int k = 0; k < 5; k++) {
         if (c->gx[k]) cudaGraphExecDestroy(c->gx[k]), c->gx[k] = nullptr;
-        if (k >= 2 && c->nh < 2) continue;   // nothing to split
+        if ((k == 2 || k == 3) && c->nh < 2) continue;   // nothing to split
         cudaGraph_t g = nullptr;
         const double lk = c->n_launches;
         cudaError_t e = cudaStreamBeginCapture(c->st_cap, cudaStreamCaptureModeThreadLocal);
         mop_status s = MOP_OK;
         if (e == cudaSuccess) {
             c->st = c->st_cap;
-            s = k == 0 ? seq_A(c, c->d_Rh) : seq_B(c, c->d_Rh, c->d_Gh, k - 1);
+            s = k == 0 ? seq_A(c, c->d_Rh) : k == 4 ? seq_A(c, c->d_Rh, false) : seq_B(c, c->d_Rh, c->d_Gh, k - 1);
             c->st = user;
             e = cudaStreamEndCapture(c->st_cap, &g);
         }
@@ -1174,6 +1175,21 @@ extern "C" mop_status mop_get_timing(mop_ctx *c, double out[16]) {
     return MOP_OK;
 }
 
+// one evaluation inside mop_step*: gradient into c->d_G; as CUDA graphs when usable (small systems are launch-bound)
+static mop_status eval_for_step(mop_ctx *c, const float *R_dev, bool deposit, bool want_energy) {
+    if (!graphs_usable(c)) return eval_async(c, R_dev, c->d_G, deposit, want_energy);
+    mop_status s = graphs_build(c);
+    if (s) return s;
+    const size_t bytes = (size_t)c->N * c->Q * 3 * sizeof(float);
+    CK(c, cudaMemcpyAsync(c->d_Rh, R_dev, bytes, cudaMemcpyDeviceToDevice, c->st));
+    CK(c, cudaGraphLaunch(c->gx[want_energy ? 0 : 4], c->st));
+    CK(c, cudaGraphLaunch(c->gx[1], c->st));
+    c->n_launches += c->gx_launches[want_energy ? 0 : 4] + c->gx_launches[1];
+    c->n_rebuilds += 1;
+    CK(c, cudaMemcpyAsync(c->d_G, c->d_Gh, bytes, cudaMemcpyDeviceToDevice, c->st));
+    return MOP_OK;
+}
+
 // velocity Verlet on eq. (4) (+ the exact OU velocity update when ou); cont: d_G already holds the gradient at R_dev
 static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pmd, int n_steps, bool cont, bool ou, double cc,
                             float amp, unsigned long long seed, unsigned long long step0) {
@@ -1185,7 +1201,7 @@ static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pm
     mop_status s;
     if (cont) {
         if (!c->g_current) FAIL(c, MOP_ERR_INVALID_ARG, "mop_step*_continue: no gradient from a previous mop_step* call is held");
-    } else if ((s = eval_async(c, R_dev, c->d_G, false, n_steps == 0))) {
+    } else if ((s = eval_for_step(c, R_dev, false, n_steps == 0))) {
         return s;
     }
     c->g_current = false;
@@ -1195,7 +1211,7 @@ static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pm
                (double *)nullptr);
         c->bias_steps += 1;
         const bool last = it == n_steps - 1;   // V_eff (mop_get_stats) is that of the last evaluation of the call: only it forms U(R^1)
-        if ((s = eval_async(c, R_dev, c->d_G, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0, last))) return s;
+        if ((s = eval_for_step(c, R_dev, c->bias_on && c->bias_pace > 0 && c->bias_steps % c->bias_pace == 0, last))) return s;
         if (last) CK(c, cudaMemsetAsync(c->d_energy + 5, 0, sizeof(double), c->st));
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (last && !ou) ? c->d_energy + 5 : (double *)nullptr);

@@ -327,10 +327,11 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             const unsigned info = __ballot_sync(0xffffffffu, (cur.y & infobit) != 0u) & 0x3fu;
             const unsigned upat = info & 15u;
             const bool shifted = (info >> 4) & 1u, masked = (info >> 5) & 1u;
-            // (the energy variant, bead 1 only, compiles the general form alone: with the FP64 reaction-field energy three
-            // copies of the step body overflow the instruction cache -- "no instruction" was its top stall reason)
-            if (ENERGY || shifted) step(cur, upat, true, true, cp, ce, tj8);
-            else if (masked) step(cur, upat, false, true, cp, ce, tj8);
+            // two compiled step bodies: the plain one (69 % of the steps on the bench workload) and the general one (periodic
+            // shift and exclusion bits).  A third, masked-only body measured the same (3.738 vs 3.734 ms per step) and the
+            // kernels are sensitive to code size: the energy variant (bead 1 only) compiles the general body alone -- with the
+            // FP64 reaction-field energy and three bodies it overflowed the instruction cache ("no instruction" 5 per issue)
+if (ENERGY || shifted || masked) step(cur, upat, true, true, cp, ce, tj8);
             else step(cur, upat, false, false, cp, ce, tj8);
         }
         mop_cp_wait<0>();

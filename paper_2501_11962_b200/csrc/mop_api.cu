@@ -938,8 +938,8 @@ static mop_status seq_B(mop_ctx *c, const float *R, float *G, int part = 0) {
     mop_status s;
     if (part == 2) {   // second group: H.eta of beads [h, nh), gradient rows [h, N)
         LAUNCH(c, nb_pick(NB_HVP), c->nb_blocks_h, 128, nb_smem(c), nb_args(c, c->d_H4, 4, 4));
-        if (G)
-            LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), N - h), 256, 0, c->Q, c->g.S, h, N, c->nh, 1, c->d_slot_of, c->d_F4,
+        if (G && N - 1 > h)   // rows [h, N-1): the last row went out with the first group
+            LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), N - 1 - h), 256, 0, c->Q, c->g.S, h, N, c->nh, 1, c->d_slot_of, c->d_F4,
                    c->d_et, c->d_H4, c->d_Ki, (const float *)nullptr, G);
         CK(c, cudaGetLastError());
         return MOP_OK;
@@ -985,9 +985,13 @@ static mop_status seq_B(mop_ctx *c, const float *R, float *G, int part = 0) {
         t_mark(c, 6);
     }
     t_mark(c, 7);
-    if (G)
+    if (G) {
         LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), part ? h : N), 256, 0, c->Q, c->g.S, 0, N, c->nh, 1, c->d_slot_of, c->d_F4,
                c->d_et, c->d_H4, c->d_Ki, (const float *)nullptr, G);
+        if (part)   // the last bead's row is K eta^{N-1} alone (eq. 7): ready now, it leaves with the first group
+            LAUNCH(c, k_assemble, dim3(cdiv(c->Q, 256), 1), 256, 0, c->Q, c->g.S, N - 1, N, c->nh, 1, c->d_slot_of, c->d_F4,
+                   c->d_et, c->d_H4, c->d_Ki, (const float *)nullptr, G);
+    }
     t_mark(c, 8);
     CK(c, cudaGetLastError());
     return MOP_OK;
@@ -1083,12 +1087,15 @@ extern "C" mop_status mop_eval_veff_grad_host(mop_ctx *c, const float *R_host, d
         CK(c, cudaEventRecord(c->ev_copy[3], c->st));
         CK(c, cudaStreamWaitEvent(c->st_copy, c->ev_copy[3], 0));
         CK(c, cudaMemcpyAsync(grad_host, G, h * bead * sizeof(float), cudaMemcpyDeviceToHost, c->st_copy));
+        CK(c, cudaMemcpyAsync(grad_host + (size_t)(N - 1) * bead, G + (size_t)(N - 1) * bead, bead * sizeof(float),
+                              cudaMemcpyDeviceToHost, c->st_copy));   // the last row (eq. 7) is complete already
         CK(c, cudaEventRecord(c->ev_copy[0], c->st_copy));
         if (graphs) CK(c, cudaGraphLaunch(c->gx[3], c->st));
         else if ((s = seq_B(c, R, G, 2))) return s;
         if (graphs) c->n_launches += c->gx_launches[0] + c->gx_launches[2] + c->gx_launches[3];
-        CK(c, cudaMemcpyAsync(grad_host + h * bead, G + h * bead, ((size_t)N - h) * bead * sizeof(float), cudaMemcpyDeviceToHost,
-                              c->st));
+        if ((size_t)N - 1 > h)
+            CK(c, cudaMemcpyAsync(grad_host + h * bead, G + h * bead, ((size_t)N - 1 - h) * bead * sizeof(float),
+                                  cudaMemcpyDeviceToHost, c->st));
         CK(c, cudaStreamWaitEvent(c->st, c->ev_copy[0], 0));   // the final synchronisation of st covers both copies
     }
     c->n_rebuilds += 1;

@@ -621,6 +621,25 @@ def test_one_context_different_paths_in_turn(B, oracle):
     m.close()
 
 
+def test_topology_can_be_replaced(B, oracle):
+    """mop_set_topology again on a live context (here: all charges zero): captured graphs and lists follow."""
+    import copy
+    s, o, R = case(oracle, "c2")
+    m = B.Mop(s, s.n_beads)
+    v0, _ = m.mop_eval_veff_grad(R)
+    v0b, _ = m.mop_eval_veff_grad(R)                      # graph replay
+    s2 = copy.copy(s)
+    s2.charge = np.zeros_like(s.charge)
+    m.mop_set_topology(s2)
+    v1, g1 = m.mop_eval_veff_grad(R)
+    v1b, g1b = m.mop_eval_veff_grad(R)
+    v_ref, g_ref = oracle.veff_grad(oracle.OracleSystem(s2), R.astype(np.float64), geom=1, brute=False)
+    assert abs(v0 - v0b) <= 1e-7 * abs(v0) and abs(v1 - v_ref) <= TOL_V * abs(v_ref) and abs(v1b - v_ref) <= TOL_V * abs(v_ref)
+    assert abs(v1 - v0) > 1e-3 * abs(v0)
+    H.assert_close(g1b.cpu().numpy(), g_ref, TOL_RMS)
+    m.close()
+
+
 def test_argument_errors_of_the_added_entry_points(B):
     import torch
     s = W.config1(n_beads=1)

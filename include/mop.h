@@ -224,10 +224,13 @@ mop_status mop_step_langevin_continue(mop_ctx *c, float *R_dev, float *V_dev, do
 
 /* The production force kernel's OWN in-range decisions over the pair list of the last evaluation: its counting
  * instance (the same code plus a population count of the per-pair results of the predicate G8 and of the exclusion
- * masks) is run once more and the count returned in HOST *n_inrange.  which = 0: bead 1; 1: the other force beads;
- * 2: all force beads.  This, not the scalar walker of mop_debug_pairs, is what the bit-exact neighbour-set claim of
- * the pair kernels rests on (the tests hold it equal to the oracle's pair count).  Synchronises. */
-mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange);
+ * masks) is run once more; HOST *n_inrange receives the count and *pair_hash (may be NULL) an order-independent
+ * fingerprint of the decided pair SET: the sum mod 2^64 over the decided pairs of splitmix64(((bead * Q + min(i,j)) * Q +
+ * max(i,j)) + 0x9E3779B97F4A7C15) with i, j original atom indices and bead the 0-based force bead.  which = 0: bead 1;
+ * 1: the other force beads; 2: all force beads.  This, not the scalar walker of mop_debug_pairs, is what the bit-exact
+ * neighbour-set claim of the pair kernels rests on (the tests hold count and fingerprint equal to the oracle's pair list).
+ * Synchronises. */
+mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange, unsigned long long *pair_hash);
 
 /* Testing aid: replaces the pair-list buffers by ones of the given capacities (work units, octet-pair entries, exclusion-mask
  * rows; 0 keeps one; at least 64 each) and switches off the automatic capacity check of the first evaluation, so that the

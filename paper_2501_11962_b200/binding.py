@@ -77,7 +77,7 @@ def load(build_if_missing=True):
     L.mop_get_timing.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     L.mop_step_continue.argtypes = L.mop_step.argtypes
     L.mop_step_continue.restype = C.c_int
-    L.mop_debug_count_inrange.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong)]
+    L.mop_debug_count_inrange.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong), C.POINTER(C.c_ulonglong)]
     L.mop_debug_count_inrange.restype = C.c_int
     L.mop_debug_set_list_capacity.argtypes = [C.c_void_p, C.c_uint, C.c_uint, C.c_uint]
     L.mop_debug_set_list_capacity.restype = C.c_int
@@ -373,9 +373,15 @@ class Mop:
     def mop_debug_count_inrange(self, which=2):
         """In-range, non-excluded pair decisions of the PRODUCTION force kernel (counting instance) over the list of
         the last evaluation.  which: 0 bead 1, 1 the other force beads, 2 all force beads."""
-        n = C.c_longlong(0)
-        self._check(self.L.mop_debug_count_inrange(self.ctx, int(which), C.byref(n)))
+        n, h = C.c_longlong(0), C.c_ulonglong(0)
+        self._check(self.L.mop_debug_count_inrange(self.ctx, int(which), C.byref(n), C.byref(h)))
+        self.last_pair_hash = int(h.value)
         return int(n.value)
+
+    def mop_debug_pair_hash(self, which=2):
+        """(count, fingerprint) of the production kernel's decided pair set (see mop.h)."""
+        n = self.mop_debug_count_inrange(which)
+        return n, self.last_pair_hash
 
     def mop_debug_set_list_capacity(self, units=0, entries=0, masks=0):
         self._check(self.L.mop_debug_set_list_capacity(self.ctx, int(units), int(entries), int(masks)))

@@ -618,6 +618,7 @@ static NbArgs nb_args(mop_ctx *c, float4 *out, int work_slot, int range) {
     a.cap_units = c->cap_units;
     a.cap_entries = c->cap_entries, a.cap_masks = c->cap_masks, a.n_slots = (unsigned)c->nf * (unsigned)c->g.S;
     a.n_inrange = &c->d_ctr->n_inrange;
+    a.pair_hash = &c->d_ctr->pair_hash, a.perm = c->d_perm, a.Q = c->Q;
     a.work = c->d_work + work_slot;
     a.range = range;
     a.tab = c->d_tab, a.tabs = c->d_tabs;
@@ -1433,17 +1434,18 @@ extern "C" mop_status mop_debug_pairs(mop_ctx *c, int bead, int *pairs, long lon
 // The production force kernel's own in-range decisions (its counting instance: same code, plus a population count
 // of the per-pair predicate results) over the list of the last evaluation.  which = 0: bead 1; 1: the other force
 // beads; 2: all force beads.  The forces it computes go to the H.eta scratch array.  Synchronises.
-extern "C" mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange) {
+extern "C" mop_status mop_debug_count_inrange(mop_ctx *c, int which, long long *n_inrange, unsigned long long *pair_hash) {
     PRECHECK(c);
     if (which < 0 || which > 2 || !n_inrange) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_count_inrange: bad argument");
     if (c->n_rebuilds == 0) FAIL(c, MOP_ERR_INVALID_ARG, "mop_debug_count_inrange: no evaluation yet");
-    CK(c, cudaMemsetAsync(&c->d_ctr->n_inrange, 0, sizeof(unsigned long long), c->st));
+    CK(c, cudaMemsetAsync(&c->d_ctr->n_inrange, 0, 2 * sizeof(unsigned long long), c->st));   // count and hash
     CK(c, cudaMemsetAsync(c->d_work + 3, 0, sizeof(unsigned), c->st));
     LAUNCH(c, nb_pick(NB_FORCE, true), c->nb_blocks_c, 128, nb_smem(c), nb_args(c, c->d_H4, 3, which));
     CK(c, cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaStreamSynchronize(c->st));
     CK(c, cudaGetLastError());
     *n_inrange = (long long)c->h_ctr->n_inrange;
+    if (pair_hash) *pair_hash = c->h_ctr->pair_hash;
     return MOP_OK;
 }
 

@@ -72,6 +72,7 @@ struct MopCounters {
                                                             // n_units_mid: units of the first bead group (split pass 2 of the host entry point)
     unsigned long long n_pairs;   // debug pair walker
     unsigned long long n_inrange; // in-range decisions counted by the production force kernel (counting variant)
+    unsigned long long pair_hash; // ... and the sum (mod 2^64) of a 64-bit hash of (bead, i, j) over those decisions
 };
 
 // ---- G8: the FP32 expressions shared by every kernel that classifies (fixed order, never contracted) ----

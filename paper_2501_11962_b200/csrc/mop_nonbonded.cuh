@@ -27,6 +27,9 @@ struct NbArgs {
     unsigned cap_units;              // units beyond the allocation were never written (overflow): never read them
     unsigned cap_entries, cap_masks, n_slots;   // checked build only: sizes of entries, masks and of the [nf][S] arrays
     unsigned long long *n_inrange;   // counting variant only: in-range, non-excluded pair decisions of this launch
+    unsigned long long *pair_hash;   // counting variant only: sum of mop_pair_hash over those decisions
+    const int *perm;                 // counting variant only: [nf][S] sorted slot -> original atom
+    int Q;                           // counting variant only
     unsigned *work;     // dynamic work counter (zeroed before the launch)
     int range;          // 0: units [0, n_units_bead0)   1: [n_units_bead0, n_units)   2: all   3: [0, n_units_mid)   4: [n_units_mid, n_units)
     const float2 *tab;  // [nt*nt] (6 C6, 12 C12)
@@ -34,6 +37,16 @@ struct NbArgs {
     double *energies;   // [0] U_lj, [1] U_coul
     float box[3];
 };
+
+// counting variant: order-independent fingerprint of the decided pair set.  key = (bead * Q + min(i,j)) * Q + max(i,j) in
+// original atom indices, hashed by the SplitMix64 finaliser (Steele, Lea, Flood 2014; the published constants)
+__device__ __forceinline__ unsigned long long mop_pair_hash(unsigned long long bead, unsigned long long Q, int i, int j) {
+    const unsigned long long lo = (unsigned long long)min(i, j), hi = (unsigned long long)max(i, j);
+    unsigned long long z = (bead * Q + lo) * Q + hi + 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
 
 __device__ __forceinline__ float mop_rsqrt(float x) {
     float y;

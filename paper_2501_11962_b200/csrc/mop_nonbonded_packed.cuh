@@ -106,6 +106,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         d[6] = p.w * MOP_KE;
         d[8] = e.x, d[10] = e.y, d[12] = e.z;
         d[14] = __int_as_float((int)tab6 + ti * a.nt * 8);
+        if (COUNT) d[8] = __int_as_float(a.perm[ibase + lane]);   // original index of the i atom (the eta slot is free in force mode)
         if (ENERGY) {
             asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(sd_addr + lane * 32u), "d"((double)p.x), "d"((double)p.y) : "memory");
             asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(sd_addr + lane * 32u + 16u), "d"((double)p.z),
@@ -120,6 +121,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
     for (int p = 0; p < 4; p++) ax[p] = ay[p] = az[p] = 0ull;
     double e_lj = 0.0, e_c = 0.0;
     unsigned n_in = 0;
+    unsigned long long h_in = 0ull;
     const f2 nk2rf = f2_bc(-a.k2rf);
     const unsigned lane16 = (unsigned)lane * 16u;
 
@@ -149,6 +151,7 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
         }
         // lm: bit k set iff i atom k may interact with this lane's j atom (diagonal block, exclusions)
         // (a padding entry -- pattern 0, it points at the unit's own octet -- allows nothing)
+        const int jorig = COUNT ? a.perm[cur.x + jl] : 0;   // counting variant: original index of the lane's j atom
         const bool valid = (cur.y & 15u) != 0u;
         unsigned lm = valid ? 0xffu : 0u;
         if (masked) {
@@ -173,7 +176,12 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
                 ina = ina && ((lm >> (2 * p)) & 1u);
                 inb = inb && ((lm >> (2 * p + 1)) & 1u);
             }
-            if (COUNT) n_in += (ina ? 1u : 0u) + (inb ? 1u : 0u);
+            if (COUNT) {
+                n_in += (ina ? 1u : 0u) + (inb ? 1u : 0u);
+                const float2 io = mop_lds_v2(sw_addr + p * 64 + 32);   // original indices of the two i atoms
+                if (ina) h_in += mop_pair_hash((unsigned long long)un.bead, (unsigned long long)a.Q, __float_as_int(io.x), jorig);
+                if (inb) h_in += mop_pair_hash((unsigned long long)un.bead, (unsigned long long)a.Q, __float_as_int(io.y), jorig);
+            }
             const float ra = mop_rsqrt(r2a), rb = mop_rsqrt(r2b);
             const f2 rinv = f2_pack(ra, rb);
             const f2 qq = f2_mul(Qi, jq);
@@ -371,6 +379,9 @@ if (ENERGY || shifted || masked) step(cur, upat, true, true, cp, ce, tj8);
     if (COUNT) {
         n_in = (unsigned)__reduce_add_sync(0xffffffffu, n_in);
         if (lane == 0) atomicAdd(a.n_inrange, (unsigned long long)n_in);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) h_in += __shfl_xor_sync(0xffffffffu, h_in, o);
+        if (lane == 0) atomicAdd(a.pair_hash, h_in);
     }
 }
 

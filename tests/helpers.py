@@ -101,3 +101,19 @@ def assert_close(a, b, tol_rms, tol_max=TOL_MAX):
     k = np.unravel_index(excess.argmax(), excess.shape)
     assert excess[k] <= 0, "|delta| %.3e > %.1e x rms(ref) %.3e + %.1e x |ref atom| at component %s" % (
         abs(a[k] - b[k]), tol_max, scale, tol_rms, k)
+
+
+def pair_set_fingerprint(pairs_by_bead, Q):
+    """The fingerprint mop_debug_count_inrange documents (include/mop.h), from a list of (bead index, pairs [n][2]):
+    sum mod 2^64 of splitmix64(((bead * Q + min(i,j)) * Q + max(i,j)) + 0x9E3779B97F4A7C15)."""
+    total = np.uint64(0)
+    with np.errstate(over="ignore"):
+        for bead, P in pairs_by_bead:
+            P = np.asarray(P, np.int64)
+            lo, hi = np.minimum(P[:, 0], P[:, 1]).astype(np.uint64), np.maximum(P[:, 0], P[:, 1]).astype(np.uint64)
+            z = (np.uint64(bead) * np.uint64(Q) + lo) * np.uint64(Q) + hi + np.uint64(0x9E3779B97F4A7C15)
+            z = (z ^ (z >> np.uint64(30))) * np.uint64(0xBF58476D1CE4E5B9)
+            z = (z ^ (z >> np.uint64(27))) * np.uint64(0x94D049BB133111EB)
+            z = z ^ (z >> np.uint64(31))
+            total = total + z.sum(dtype=np.uint64)
+    return int(total)

@@ -83,7 +83,7 @@ def test_config4_full_size_bench_configuration(B, oracle, big):
     assert sum(n_ref) == parts["npairs"]
     for n in range(1, m.nf):
         assert m.mop_debug_pairs(n, cap=0)[1] == n_ref[n], "pair count differs on bead %d" % n
-    assert m.mop_debug_count_inrange(0) == n_ref[0]
+    assert m.mop_debug_pair_hash(0) == (n_ref[0], H.pair_set_fingerprint([(0, ref)], s.n_atoms))   # the production kernel's own pair SET
     assert m.mop_debug_count_inrange(1) == sum(n_ref[1:])
     m.close()
 

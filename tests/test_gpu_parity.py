@@ -194,16 +194,19 @@ def test_energy_terms_of_a_single_bead(B, oracle, name):
 def test_production_kernel_inrange_count_equals_oracle_pair_count(B, oracle, name):
     """The bit-exact neighbour-set claim for the PRODUCTION force kernel (not the scalar pair walker): its counting
     instance -- the same code plus a population count of its own per-pair decisions (G8 predicate AND exclusion bit) --
-    must count exactly the oracle's in-range, non-excluded pairs, bead 1 and the other force beads separately.  The
-    walker's pair SET is compared in test_neighbour_sets_bit_exact; equal counts over a list that holds every pair
-    at most once leave no room for a differing decision."""
+    must count exactly the oracle's in-range, non-excluded pairs, bead 1 and the other force beads separately, and its
+    fingerprint of the decided pairs (a 64-bit hash of (bead, i, j) summed over them) must equal the fingerprint of the
+    oracle's pair lists: the same set, not only the same size."""
     s, o, R = case(oracle, name)
     m = B.Mop(s, s.n_beads)
     m.mop_eval_veff_grad(R, want_grad=False)
-    n_ref = [oracle.bead(o, R[n].astype(np.float64), geom=1, want_force=False)["npairs"] for n in range(m.nf)]
+    P = [oracle.pairs(o, R[n].astype(np.float64), geom=1, brute=s.n_atoms <= 3000) for n in range(m.nf)]
+    n_ref = [len(p) for p in P]
     assert m.mop_debug_count_inrange(0) == n_ref[0]
     assert m.mop_debug_count_inrange(1) == sum(n_ref[1:])
-    assert m.mop_debug_count_inrange(2) == sum(n_ref)
+    # ... and the SET: the kernel's order-independent 64-bit fingerprint of (bead, i, j) over its own decisions
+    assert m.mop_debug_pair_hash(2) == (sum(n_ref), H.pair_set_fingerprint(list(enumerate(P)), s.n_atoms))
+    assert m.mop_debug_pair_hash(0) == (n_ref[0], H.pair_set_fingerprint([(0, P[0])], s.n_atoms))
     m.close()
 
 

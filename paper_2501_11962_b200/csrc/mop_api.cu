@@ -148,8 +148,12 @@ static inline unsigned cdiv(size_t a, size_t b) { return (unsigned)((a + b - 1) 
 typedef void (*nb_kernel_t)(const NbArgs);
 // the launched instances of the pair kernel: six resident CTAs per SM (80 registers) for the force passes, five (96)
 // for the H.eta pass (measured: profiles/r02_experiments.md)
+#ifndef NBP_CTAS_F
 #define NBP_CTAS_F 6
+#endif
+#ifndef NBP_CTAS_H
 #define NBP_CTAS_H 5
+#endif
 #define NBP_CTAS_E 4   // energy variant (bead 1 only): FP64 sums and six more packed accumulators per step
 static nb_kernel_t nb_pick(int mode, bool count = false) {
     if (count) return k_nonbonded_p<NB_FORCE, true, NBP_CTAS_F>;

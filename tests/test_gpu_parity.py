@@ -624,6 +624,28 @@ def test_one_context_different_paths_in_turn(B, oracle):
     m.close()
 
 
+@pytest.mark.parametrize("name", ["lj_n1", "lj_n2", "chain", "c3"])
+def test_graph_replay_and_host_entry_point_at_small_bead_counts(B, oracle, name):
+    """The first evaluation of a context takes the plain launch sequence (it checks the list capacities); later ones replay
+    the CUDA graphs, and the host entry point splits its copies only when there are at least two H.eta beads: N = 1, 2, 3
+    and 6 through all three forms against the oracle."""
+    import torch
+    s, o, R = case(oracle, name)
+    v_ref, g_ref = oracle.veff_grad(o, R.astype(np.float64), geom=1, brute=s.n_atoms <= 3000)
+    m = B.Mop(s, s.n_beads)
+    Rh, Gh = torch.as_tensor(R).pin_memory(), torch.empty(R.shape, dtype=torch.float32).pin_memory()
+    for form in ("first", "graphs", "graphs", "host", "host"):
+        if form == "host":
+            v = m.mop_eval_veff_grad_host(Rh, Gh)
+            g = Gh.numpy().copy()
+        else:
+            v, g = m.mop_eval_veff_grad(R)
+            g = g.cpu().numpy()
+        assert abs(v - v_ref) <= TOL_V * abs(v_ref), form
+        H.assert_close(g, g_ref, TOL_RMS)
+    m.close()
+
+
 def test_topology_can_be_replaced(B, oracle):
     """mop_set_topology again on a live context (here: all charges zero): captured graphs and lists follow."""
     import copy

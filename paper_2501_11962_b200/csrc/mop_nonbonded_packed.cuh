@@ -336,10 +336,10 @@ __device__ __forceinline__ void nbp_unit(const NbArgs &a, const MopUnit &un, flo
             const unsigned upat = info & 15u;
             const bool shifted = (info >> 4) & 1u, masked = (info >> 5) & 1u;
             // two compiled step bodies: the plain one (69 % of the steps on the bench workload) and the general one (periodic
-            // shift and exclusion bits).  A third, masked-only body measured the same (3.738 vs 3.734 ms per step) and the
-            // kernels are sensitive to code size: the energy variant (bead 1 only) compiles the general body alone -- with the
-            // FP64 reaction-field energy and three bodies it overflowed the instruction cache ("no instruction" 5 per issue)
-if (ENERGY || shifted || masked) step(cur, upat, true, true, cp, ce, tj8);
+            // shift and exclusion bits).  A third, masked-only body measured the same (3.738 vs 3.734 ms per step), and the
+            // kernels are sensitive to code size: with FP64 LJ and reaction-field energies and three bodies the energy variant
+            // (4,500 instructions) overflowed the instruction cache ("no instruction" 5 stalls per issue)
+            if (shifted || masked) step(cur, upat, true, true, cp, ce, tj8);
             else step(cur, upat, false, false, cp, ce, tj8);
         }
         mop_cp_wait<0>();

@@ -362,7 +362,9 @@ def run_ours(a):
                    "path": "Brownian recursion, dt=2 fs, nu=50/ps, T=%g K, seed %d" % (s.temperature, rank)},
         "pair_interactions_per_sec": (pairs_force_job + pairs_hvp_job) / (ms_per_step * 1e-3),
         "pairs_in_range_per_bead": pairs_force / max(m.nf, 1),
-        "pair_slots_evaluated_per_pass": st1["pair_slots"],
+        "pair_slots_admitted_by_patterns_per_pass": st1["pair_slots"],
+        "pair_slots_evaluated_per_pass": st1["pair_slots_evaluated"],
+        "evaluated_slots_per_in_range_pair": st1["pair_slots_evaluated"] / max(pairs_force, 1.0),
         "stage_ms": {k: round(v, 5) for k, v in stages.items() if k != "evals"},
         "roofline": {"bound": "alu", "kernel": "k_nonbonded<HVP> (S5, fused force-scalar + H.eta pair kernel)",
                      "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,

@@ -134,7 +134,8 @@ const char *mop_last_error(const mop_ctx *c);
  * [6]=U_angle(R^1), [7]=kinetic energy after the last mop_step, [8]=pair-list rebuilds so far,
  * [9]=cluster-pair entries in the current list, [10]=list units, [11]=exclusion masks,
  * [12]=pair slots the list admits per nonbonded pass (sum over entries of popcount(row-pair pattern) * 16), [13]=kernel launches so far,
- * [14]=evaluations that reused a buffered list (r_buf > 0), [15] reserved. */
+ * [14]=evaluations that reused a buffered list (r_buf > 0), [15]=pair slots the pair kernels evaluate per pass (64 per row pair
+ * of every step's union pattern: [12] plus the steps whose four octets differ in pattern). */
 mop_status mop_get_stats(mop_ctx *c, double out[16]);
 
 /* Stage timing with CUDA events on the context stream (the stream the kernels are launched on).  on != 0: every

@@ -339,8 +339,8 @@ class Mop:
         out = (C.c_double * 16)()
         self._check(self.L.mop_get_stats(self.ctx, out))
         k = ["veff", "U1", "E_spring", "U_lj", "U_coul", "U_bond", "U_angle", "E_kin", "rebuilds", "entries", "units",
-             "masks", "pair_slots", "launches", "reuses"]
-        return dict(zip(k, list(out)[:15]))
+             "masks", "pair_slots", "launches", "reuses", "pair_slots_evaluated"]
+        return dict(zip(k, list(out)[:16]))
 
     def dims(self):
         d = np.zeros(8, np.int32)

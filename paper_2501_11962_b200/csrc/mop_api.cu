@@ -309,12 +309,12 @@ static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int 
     A(dalloc(&c->d_blo, nf * S / MOP_CL));
     A(dalloc(&c->d_bhi, nf * S / MOP_CL));
     A(dalloc(&c->d_ctr, 1));
-    A(dalloc(&c->d_slots, 1));
+    A(dalloc(&c->d_slots, 2));
     A(dalloc(&c->d_work, 8));
     A(dalloc(&c->d_energy, 16));   // [0..5] U_lj, U_coul, U_bond, U_angle, E_spring, E_kin; [8..15] scratch
     A(cudaMallocHost((void **)&c->h_energy, 8 * sizeof(double)));
     A(cudaMallocHost((void **)&c->h_ctr, sizeof(MopCounters)));
-    A(cudaMallocHost((void **)&c->h_slots, sizeof(unsigned long long)));
+    A(cudaMallocHost((void **)&c->h_slots, 2 * sizeof(unsigned long long)));
     A(cudaStreamCreateWithFlags(&c->st2, cudaStreamNonBlocking));
     A(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     A(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
@@ -331,10 +331,10 @@ static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int 
     }
     cudaMemsetAsync(c->d_energy, 0, 16 * sizeof(double), c->st);
     cudaMemsetAsync(c->d_ctr, 0, sizeof(MopCounters), c->st);
-    cudaMemsetAsync(c->d_slots, 0, sizeof(unsigned long long), c->st);
+    cudaMemsetAsync(c->d_slots, 0, 2 * sizeof(unsigned long long), c->st);
     memset(c->h_energy, 0, 8 * sizeof(double));
     memset(c->h_ctr, 0, sizeof(MopCounters));
-    *c->h_slots = 0;
+    c->h_slots[0] = c->h_slots[1] = 0;
     *out = c;
     return MOP_OK;
 }
@@ -526,7 +526,7 @@ static void t_mark(mop_ctx *c, int k) {
 // per-build counters start from zero; the overflow and non-finite words are sticky (only a regrow clears overflow)
 __global__ void k_ctr_reset(MopCounters *ctr, unsigned long long *slots) {
     ctr->n_units = ctr->n_entries = ctr->n_masks = ctr->n_units_bead0 = ctr->n_units_mid = 0u;
-    *slots = 0ull;
+    slots[0] = slots[1] = 0ull;
 }
 __global__ void k_ctr_clear_overflow(MopCounters *ctr) { ctr->overflow = 0u; }
 
@@ -692,7 +692,7 @@ static mop_status pass_hvp(mop_ctx *c, const float *R, int nb, bool timed = fals
 static mop_status read_back(mop_ctx *c) {
     CK(c, cudaMemcpyAsync(c->h_energy, c->d_energy, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaMemcpyAsync(c->h_ctr, c->d_ctr, sizeof(MopCounters), cudaMemcpyDeviceToHost, c->st));
-    CK(c, cudaMemcpyAsync(c->h_slots, c->d_slots, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->st));
+    CK(c, cudaMemcpyAsync(c->h_slots, c->d_slots, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->st));
     CK(c, cudaStreamSynchronize(c->st));
     CK(c, cudaGetLastError());
     if (c->h_ctr->nonfinite) {
@@ -1374,7 +1374,7 @@ extern "C" mop_status mop_get_stats(mop_ctx *c, double out[16]) {
     out[12] = (double)(*c->h_slots);
     out[13] = c->n_launches;
     out[14] = c->n_reuses;
-    out[15] = 0.0;
+    out[15] = (double)c->h_slots[1];
     return MOP_OK;
 }
 

@@ -26,7 +26,7 @@ struct PlArgs {
     MopEntry *entries;
     unsigned long long *masks;
     MopCounters *ctr;
-    unsigned long long *slots_active; // sum over entries of popc(pattern) * 16
+    unsigned long long *slots_active; // [0] sum over entries of popc(pattern) * 16; [1] sum over steps of popc(union pattern) * 64
     unsigned cap_units, cap_entries, cap_masks;
 };
 
@@ -393,6 +393,7 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
         }
         if (lane < (int)(padded - total)) sorted[total + lane] = make_uint2((unsigned)ci | ((unsigned)MOP_NOSHIFT << 24), 0u);
         __syncwarp();
+        unsigned nunion = 0;   // pair slots the pair kernels evaluate: 64 per row pair of every step's union pattern
         for (unsigned sidx = lane; sidx < padded / MOP_NG; sidx += 32) {
             uint2 e[MOP_NG];
             unsigned u = 0, fl = 0;
@@ -404,14 +405,17 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
                 if ((e[q].y >> 8) != 0u || (e[q].y & 15u) == 0u) fl |= 1u << 21;
             }
             fl |= u << 16;
+            nunion += __popc(u) * 64u;
             MOP_ASSERT(st + (sidx + 1) * MOP_NG <= a.cap_entries && (st % MOP_NG) == 0);
             uint4 *dst = reinterpret_cast<uint4 *>(a.entries + st + sidx * MOP_NG); // st is a multiple of 4: 32 B aligned
             dst[0] = make_uint4(e[0].x, e[0].y | fl, e[1].x, e[1].y | fl);
             dst[1] = make_uint4(e[2].x, e[2].y | fl, e[3].x, e[3].y | fl);
         }
+        nunion = (unsigned)__reduce_add_sync(0xffffffffu, nunion);
         if (lane == 0) {
             MopUnit un = {n, ci, st, padded, mb, 0u, 0u, 0u};
             a.units[ui] = un;
+            atomicAdd(a.slots_active + 1, (unsigned long long)nunion);
         }
         } while (false);
     }

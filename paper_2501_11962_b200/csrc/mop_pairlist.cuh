@@ -35,9 +35,10 @@ __device__ __forceinline__ float mop_gap(float lo_a, float hi_a, float lo_b, flo
     return fmaxf(0.0f, fmaxf(lo_b - hi_a, lo_a - hi_b));
 }
 
-// bucket order of the 15 non-zero patterns: full first, then the contiguous runs (the usual partial patterns, the
-// row pairs of an octet being ordered along z), then the rest
-__constant__ unsigned char c_pat_order[16] = {15, 7, 3, 1, 14, 12, 8, 6, 2, 4, 5, 9, 10, 11, 13, 0};
+// bucket order of the 15 non-zero patterns: the contiguous runs (the usual patterns, the row pairs of an octet being
+// ordered along z) as a chain in which neighbours differ by one row pair -- 1, 3, 7, 15, 14, 12, 8 -- so that a step of four
+// entries that straddles two buckets evaluates at most one row pair too many; then the rest
+__constant__ unsigned char c_pat_order[16] = {1, 3, 7, 15, 14, 12, 8, 6, 2, 4, 5, 9, 10, 11, 13, 0};
 
 #define MOP_PL_WARPS 4     // warps (i-octets) per CTA of the list builder
 #ifndef MOP_PL_MINB
@@ -326,10 +327,12 @@ __global__ void __launch_bounds__(32 * MOP_PL_WARPS, MOP_PL_MINB) k_pairlist(PlA
         }
         __syncwarp();
 
-        // ---- bucket starts in (pattern order, plain before shifted), total, padded total
+        // ---- bucket starts: the 15 plain buckets in pattern order, then the 15 shifted ones in reverse pattern order (one
+        // junction between plain and shifted entries, and between equal patterns: few steps take the general body for a
+        // single shifted entry), total, padded total
         unsigned mycnt = 0, mykey = 0;
         if (lane < 30) {
-            mykey = (unsigned)c_pat_order[lane >> 1] | ((lane & 1) << 4);
+            mykey = lane < 15 ? (unsigned)c_pat_order[lane] : ((unsigned)c_pat_order[29 - lane] | 16u);
             mycnt = pcnt[mykey];
         }
         unsigned incl = mycnt;

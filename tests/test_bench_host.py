@@ -50,3 +50,14 @@ def test_reference_arm_other_ranks_exit_without_work():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        capture_output=True, text=True, timeout=120, env=env)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_roofline_traffic_comes_from_the_committed_ncu_capture():
+    """roofline.traffic is read from profiles/ (the ncu capture of the S5 launch), not typed into bench.py."""
+    sys.path.insert(0, ROOT)
+    import bench
+    traffic, src = bench.traffic_bytes_per_launch()
+    assert src == bench.NCU_METRICS_FILE and os.path.exists(os.path.join(ROOT, src))
+    vals = dict(l.strip().split(",") for l in open(os.path.join(ROOT, src)) if not l.startswith("#"))
+    assert traffic == float(vals["dram__bytes_read.sum"]) + float(vals["dram__bytes_write.sum"])
+    assert 1.0e7 < traffic < 1.0e10          # bytes per launch: tens to hundreds of MB

@@ -323,13 +323,15 @@ def run_ours(a):
     n_e2e = max(3, min(a.steps, 10))
     if world > 1:
         torch.distributed.barrier()
-    torch.cuda.synchronize()
-    te = time.perf_counter()
+    # every call is host-synchronous (it returns V_eff), so its wall-clock time IS the end-to-end time of one step; the L2
+    # flush runs, and is waited for, before the clock starts
+    e2e_ms = 0.0
     for _ in range(n_e2e):
         flush.zero_()
+        torch.cuda.synchronize()
+        te = time.perf_counter()
         v_e2e = e2e_step()
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - te) * 1e3
+        e2e_ms += (time.perf_counter() - te) * 1e3
     e2e_ms_max, e2e_units = all_reduce_max_sum(e2e_ms, float(Rd.shape[0] * n_e2e), world, dev)
     if not blocks_mode and not (np.isfinite(v_e2e) and abs(v_e2e - st1["veff"]) <= 1e-5 * abs(st1["veff"])):
         raise RuntimeError("host-buffer evaluation disagrees with the device-buffer one: %r vs %r" % (v_e2e, st1["veff"]))

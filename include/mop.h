@@ -267,6 +267,39 @@ mop_status mop_block_assemble(mop_ctx *c, const float *keta_left_dev, double *ve
  * v += dt/2 (-grad)/m.  Works on any context. */
 mop_status mop_block_integrate(mop_ctx *c, float *R_dev, float *V_dev, const float *grad_dev, double dt_pmd, int stage);
 
+/* ---- for callers that must not allocate device memory ------------------------------------------------------------------
+ * Everything above works on a context, and a context allocates (mop_create, mop_set_topology, list regrowth).  Some callers
+ * cannot accept that: a host program that hands out all device memory from its own pool at start-up and forbids driver
+ * allocations afterwards, a process in which another framework has already reserved almost all of HBM, or a stepping loop
+ * that cannot afford the device-wide synchronisation of cudaMalloc / cudaFree.  For them, ONE stage of the path is offered
+ * as a stateless call that allocates nothing, neither directly nor through a library routine: the displacement and spring-
+ * energy stage S4 (the paper's PMD kernels 1 and 7)
+ *     eta^n_i = (R^{n+1}_i - R^n_i) - dt/(m_i nu) F^n_i,    E_spring = sum_{n=1}^{N-1} sum_i m_i nu/(4 dt) |eta^n_i|^2
+ * (second term of eq. (3); L^n as in reading G1), with the arithmetic of the context path (FP32 eta, FP64 sum).
+ *   device, stream   CUDA ordinal and cudaStream_t (NULL: legacy default stream) the work is enqueued on; asynchronous
+ *   R_dev            DEVICE [n_beads][n_atoms][3] float, image-consistent beads, n_beads >= 2
+ *   F_dev            DEVICE [n_beads-1][n_atoms][3] float, physical forces F^n of beads 1..N-1 (e.g. from the caller's engine)
+ *   mass_dev         DEVICE [n_atoms] float, > 0
+ *   eta_dev          DEVICE [n_beads-1][n_atoms][3] float, written
+ *   e_spring_dev     DEVICE double, written (kJ/mol); summed in a fixed order, so equal inputs give equal bits
+ *   err, err_len     HOST buffer for a message on failure (may be NULL / 0)
+ * All five device buffers belong to the caller.  The kernel's only working memory (one FP64 partial sum per 256 (atom, bead)
+ * pairs and a counter) is a fixed array of MOP_NOALLOC_SCRATCH_BYTES inside the library image; every GPU this process uses
+ * the library on holds it until exit.  Consequences the caller must know:
+ *   - size limit: n_atoms * (n_beads - 1) <= MOP_NOALLOC_MAX_ATOM_BEADS, otherwise MOP_ERR_INVALID_ARG and nothing is
+ *     launched (evaluate a longer path as consecutive bead ranges and add the energies);
+ *   - one array per device for all threads and streams: calls that may run on the same GPU at the same time race on it;
+ *     keep them on one stream or order them with events.  The call itself resets what has to start at zero, so nothing
+ *     carries over from one call to the next;
+ *   - the first call on each device looks up the array's device address (with `device` made current for the duration of
+ *     the call, restored afterwards); issue that first call outside any stream capture.
+ * Errors: INVALID_ARG (sizes, NULL pointers, dt_path or nu <= 0, limit exceeded), CUDA (no device, launch failure). */
+#define MOP_NOALLOC_MAX_ATOM_BEADS 33554432              /* 2^25 = 131,072 thread blocks of 256 */
+#define MOP_NOALLOC_SCRATCH_BYTES (256 + 131072 * 8)     /* 1,048,832 bytes per GPU */
+mop_status mop_eta_spring_noalloc(int device, void *stream, int n_atoms, int n_beads, double dt_path, double nu,
+                                  const float *R_dev, const float *F_dev, const float *mass_dev, float *eta_dev,
+                                  double *e_spring_dev, char *err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,7 +20,9 @@ EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "
            "mop_set_timing", "mop_get_timing", "mop_eval_veff_grad_fd", "mop_step_continue",
            "mop_step_langevin_continue", "mop_debug_count_inrange", "mop_create_block", "mop_block_pass1",
            "mop_block_pass2", "mop_block_assemble", "mop_block_integrate", "mop_debug_set_list_capacity",
-           "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias"]
+           "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias",
+           "mop_eta_spring_noalloc"]
+MOP_NOALLOC_MAX_ATOM_BEADS = 33554432   # include/mop.h
 
 
 class MopError(RuntimeError):
@@ -106,6 +108,9 @@ def load(build_if_missing=True):
     L.mop_add_hill.restype = C.c_int
     L.mop_get_bias.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.c_void_p, C.c_int, C.POINTER(C.c_int)]
     L.mop_get_bias.restype = C.c_int
+    L.mop_eta_spring_noalloc.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]
+    L.mop_eta_spring_noalloc.restype = C.c_int
     for n in ("mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "mop_get_stats", "mop_debug_get",
               "mop_debug_pairs", "mop_force_hvp", "mop_eval_veff_grad_host", "mop_set_timing", "mop_get_timing"):
         getattr(L, n).restype = C.c_int
@@ -129,6 +134,32 @@ def mop_probe_fp32(device=0):
 
 def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def mop_eta_spring_noalloc(R, F, mass, dt_path, nu, eta_out, e_spring_out, stream=None):
+    """eta^n and the spring energy (stage S4) for callers that must not allocate device memory: no context, and the
+    library allocates nothing -- its working memory is a fixed array inside the library image (see include/mop.h for
+    who needs this, the size limit MOP_NOALLOC_MAX_ATOM_BEADS and the rule against concurrent calls on one GPU).
+    Every tensor is the caller's, already on the GPU: R [N][Q][3], F [N-1][Q][3], mass [Q] float32; eta_out
+    [N-1][Q][3] float32 and e_spring_out (one float64) are written.  Nothing is allocated here either: the arguments
+    are passed through as they are, so they must be contiguous.  Asynchronous on `stream` (default: torch's current)."""
+    import torch
+    L = load()
+    N, Q = int(R.shape[0]), int(R.shape[1])
+    for t, shape, dt in ((R, (N, Q, 3), torch.float32), (F, (N - 1, Q, 3), torch.float32), (mass, (Q,), torch.float32),
+                         (eta_out, (N - 1, Q, 3), torch.float32), (e_spring_out, None, torch.float64)):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt and t.device == R.device):
+            raise ValueError("mop_eta_spring_noalloc takes contiguous CUDA tensors on one device (float32; energy float64)")
+        if shape is not None and tuple(t.shape) != shape:
+            raise ValueError("shape %s, expected %s" % (tuple(t.shape), shape))
+    if e_spring_out.numel() != 1:
+        raise ValueError("e_spring_out holds one float64")
+    st = stream if stream is not None else torch.cuda.current_stream(R.device)
+    err = C.create_string_buffer(512)
+    s = L.mop_eta_spring_noalloc(R.device.index or 0, C.c_void_p(st.cuda_stream), Q, N, float(dt_path), float(nu), _ptr(R),
+                                 _ptr(F), _ptr(mass), _ptr(eta_out), _ptr(e_spring_out), err, len(err))
+    if s != MOP_OK:
+        raise MopError(s, err.value.decode())
 
 
 def _np(a, dtype, shape=None):

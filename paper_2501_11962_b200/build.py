@@ -29,8 +29,11 @@ def build(force=False, verbose=False, extra=()):
     if not (force or needs_build()):
         return LIB
     flags = [f for f in FLAGS if not f.startswith("--use_fast_math")]
-    for lib, src in ((LIB, "mop_api.cu"), (PROBE_LIB, "mop_probe.cu")):
-        cmd = [NVCC] + flags + list(extra) + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib, os.path.join(CSRC, src)]
+    # mop_noalloc.cu is a translation unit of its own: its file-scope device array and the host code that looks up the
+    # array's address have to live in one file
+    for lib, srcs in ((LIB, ("mop_api.cu", "mop_noalloc.cu")), (PROBE_LIB, ("mop_probe.cu",))):
+        cmd = ([NVCC] + flags + list(extra) + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib]
+               + [os.path.join(CSRC, src) for src in srcs])
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)

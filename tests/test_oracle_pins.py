@@ -624,3 +624,160 @@ def test_geom1_matches_geom0_physics(oracle):
     v1, G1 = oracle.veff_grad(o, R32, geom=1, brute=False)
     assert v1 == pytest.approx(v0, rel=1e-12)
     assert H.rms_rel(G1, G0) < 1e-10
+
+
+# ---------------------------------------------------------------- G8 edge branches (the cases bit-exact neighbour sets turn on)
+def _wrap_by_hand(x, L):
+    """The G8 wrap written out in numpy float32 scalars (every operation rounds to single precision).
+    Returns (xw, took_negative_fixup, took_upper_fixup)."""
+    x, L = np.float32(x), np.float32(L)
+    invL = np.float32(1.0) / L
+    t = x * invL
+    f = np.floor(t)
+    p = L * f
+    xw = x - p
+    lo = bool(xw < np.float32(0.0))
+    if lo:
+        xw = xw + L
+    hi = bool(xw >= L)
+    if hi:
+        xw = xw - L
+    return np.float32(xw), lo, hi
+
+
+def test_G8_wrap_edge_inputs_stay_in_the_box(oracle):
+    """What the mathematics fixes for a periodic box: the wrapped coordinate lies in [0, L) -- L itself
+    excluded, or the cell index below would reach n -- and is the same point modulo L.  The inputs sit on and next to the
+    box faces and their periodic copies, where x * (1/L) rounds onto an integer although x does not, so that
+    x - L floor(x / L) comes out negative, or equal to L: both fix-ups of the G8 sequence are needed, and the test checks
+    that it has inputs that take each of them (it cannot go vacuous)."""
+    took_lo = took_hi = 0
+    for L in (2.88, 3.10, 10.5, 13.5):
+        Lf = np.float32(L)
+        xs = [np.float32(-1e-9), np.float32(-0.0), Lf, np.nextafter(Lf, np.float32(0)), np.nextafter(Lf, np.float32(np.inf)),
+              np.float32(1e6) * Lf, np.float32(-1e6) * Lf]
+        for k in range(-3, 4):
+            e = np.float32(k) * Lf
+            x = e
+            for _ in range(3):
+                x = np.nextafter(x, np.float32(-np.inf))
+                xs.append(x)
+            x = e
+            for _ in range(3):
+                x = np.nextafter(x, np.float32(np.inf))
+                xs.append(x)
+            xs.append(e)
+        X = np.zeros((len(xs), 3), np.float32)
+        X[:, 0] = xs
+        xw = oracle.wrap(X, [L, 5.0, 5.0])[:, 0]
+        assert (xw >= 0).all() and (xw < Lf).all(), (L, X[~((xw >= 0) & (xw < Lf)), 0])
+        for x, w in zip(xs, xw):
+            hand, lo, hi = _wrap_by_hand(x, L)
+            took_lo += lo
+            took_hi += hi
+            assert w.tobytes() == hand.tobytes() or (w == 0 and hand == 0), (L, x, w, hand)
+            # the same point modulo L: distance to the nearest periodic copy of x, within the rounding of |x| / L turns
+            d = (float(w) - float(x)) / float(Lf)
+            assert abs(d - round(d)) * float(Lf) <= 4 * np.spacing(np.float32(max(abs(float(x)), float(Lf)))), (L, x, w)
+    assert took_lo >= 1 and took_hi >= 1, (took_lo, took_hi)
+
+
+def test_G8_cell_index_of_the_last_representable_coordinate(oracle):
+    """xw = nextafter(L, 0) is inside the box, so its cell is the last one, n - 1; but xw * (n / L) can round up to n in
+    FP32, and the index n would address the first bin of the next column.  The test looks for such (L, n) among the box
+    lengths and bin counts of the configs, requires that it found some, and checks the oracle's cell ids there."""
+    found = 0
+    for L in (2.88, 3.10, 10.5, 13.5, 6.2):
+        Lf = np.float32(L)
+        xw = np.nextafter(Lf, np.float32(0))
+        for n in list(range(1, 200)) + [256, 512, 1024, 2048, 4096]:
+            sc = np.float32(n) * (np.float32(1.0) / Lf)
+            if int(xw * sc) < n:
+                continue
+            found += 1
+            X = np.array([[0.5, 0.5, xw], [xw, 0.5, 0.5]], np.float32)
+            dims = [n if n <= 1024 else 1, 1, n]
+            box = [L if n <= 1024 else 5.0, 5.0, L]
+            cell = oracle.cell_ids(X, box, dims)
+            cx0 = int(np.float32(0.5) * (np.float32(dims[0]) * (np.float32(1.0) / np.float32(box[0]))))
+            assert cell[0] == (cx0 * 1 + 0) * n + (n - 1), (L, n, cell)
+            if n <= 1024:
+                cz1 = int(np.float32(0.5) * sc)
+                assert cell[1] == ((n - 1) * 1 + 0) * n + cz1, (L, n, cell)
+    assert found >= 3, found
+
+
+@pytest.mark.parametrize("rc", [1.0, 1.5])
+def test_G8_strict_inequality_at_exactly_r_cut(oracle, rc):
+    """The cutoff test is r2 < r_c^2, strictly (reading G8).  With r_c = 1 or 1.5 and separations that are exact
+    binary fractions, r2 == r_c^2 can be hit exactly in FP32: that pair is NOT listed, the pair one ulp closer is, the pair
+    one ulp farther is not -- along each axis, in both atom orders, inside the box (k = 0) and across a face (k = +-1)."""
+    L = 4.0                                     # exact in FP32, >= 2 r_c
+
+    def n_pairs(xi, xj, axis):
+        X = np.full((2, 3), 0.5, np.float32)
+        X[0, axis], X[1, axis] = xi, xj
+        s = H.make_system("two", [L] * 3, X.astype(np.float64), [12.0, 12.0], [0.0, 0.0], [0, 0], [0.3], [0.5], r_cut=rc)
+        o = oracle.OracleSystem(s)
+        out = []
+        for Xo in (X, X[::-1].copy()):
+            a = len(oracle.pairs(o, Xo.astype(np.float64), geom=1, brute=True))
+            assert a == len(oracle.pairs(o, Xo.astype(np.float64), geom=1, brute=False))
+            out.append(a)
+        assert out[0] == out[1]
+        return out[0]
+
+    f = np.float32
+    for axis in range(3):
+        # inside the box: x_i = 1, x_j = 1 + r_c (exact)
+        xi, xj = f(1.0), f(1.0 + rc)
+        assert f(xj - xi) * f(xj - xi) == f(rc) * f(rc)               # the premise: r2 == r_c^2 exactly
+        assert n_pairs(xi, xj, axis) == 0
+        assert n_pairs(xi, np.nextafter(xj, f(0)), axis) == 1
+        assert n_pairs(xi, np.nextafter(xj, f(9)), axis) == 0
+        # across the face: x_i = 0.25, x_j = 0.25 + L - r_c; d0 = -(L - r_c), k = -1, d = d0 + L = r_c exactly
+        xi, xj = f(0.25), f(0.25 + L - rc)
+        assert f(f(xi - xj) + f(L)) == f(rc)
+        assert n_pairs(xi, xj, axis) == 0
+        assert n_pairs(xi, np.nextafter(xj, f(9)), axis) == 1         # farther from x_i directly = closer through the face
+        assert n_pairs(xi, np.nextafter(xj, f(0)), axis) == 0
+
+
+def test_G8_the_two_operand_orders_differ_only_within_ulps_of_r_cut(oracle):
+    """Reading G8 forms d = (x_i - x_j) - k L; the list builder's superset test still shifts atom i first,
+    d' = (x_i - k L) - x_j.  On the whole of config 2 (4.5 million atom pairs, by hand in numpy float32) the two
+    memberships differ on at most a handful of pairs, all within a few ulp of r_c^2 -- far inside the 1e-4 relative
+    margin the builder adds to r_list^2 -- and the oracle's FP32-contract pair list is the first of the two."""
+    s = W.config2()
+    o = oracle.OracleSystem(s)
+    X = s.R1.astype(np.float32)
+    xw = oracle.wrap(X, s.box)
+    Lf = np.asarray(s.box, np.float32)
+    iu, ju = np.triu_indices(s.n_atoms, 1)
+    r2 = {}
+    for order in ("pair", "shift_i"):
+        acc = None
+        for a in (2, 1, 0):                                            # fmaf(dz,dz, fmaf(dy,dy, dx*dx)) from the inside out
+            xi, xj = xw[iu, a], xw[ju, a]
+            d0 = xi - xj
+            k = np.rint(d0 * (np.float32(1.0) / Lf[a]))
+            kL = (k * Lf[a]).astype(np.float32)                        # k in {-1,0,1}: exact
+            d = (d0 - kL) if order == "pair" else ((xi - kL) - xj)
+            r2[(order, a)] = d
+        dx, dy, dz = (r2[(order, a)].astype(np.float64) for a in (0, 1, 2))
+        inner = (dx.astype(np.float32) * dx.astype(np.float32)).astype(np.float32)
+        mid = (dy * dy + inner.astype(np.float64)).astype(np.float32)
+        r2[order] = (dz * dz + mid.astype(np.float64)).astype(np.float32)
+    rc2 = np.float32(s.r_cut) * np.float32(s.r_cut)
+    inA, inB = r2["pair"] < rc2, r2["shift_i"] < rc2
+    diff = np.nonzero(inA != inB)[0]
+    assert len(diff) <= 8, len(diff)
+    for t in diff:
+        assert abs(float(r2["pair"][t]) - float(rc2)) <= 4 * np.spacing(rc2)
+        assert abs(float(r2["shift_i"][t]) - float(rc2)) <= 4 * np.spacing(rc2)
+    assert np.abs(r2["pair"].astype(np.float64) - r2["shift_i"]).max() <= 4 * np.spacing(np.float32(Lf.max() ** 2 / 2))
+    # the oracle's list = order "pair" minus the exclusions
+    ex = {(i, int(j)) for i in range(s.n_atoms) for j in s.excl_list[s.excl_start[i]:s.excl_start[i + 1]]}
+    mine = {(int(i), int(j)) for i, j in zip(iu[inA], ju[inA])} - ex
+    ref = {(int(i), int(j)) for i, j in oracle.pairs(o, X.astype(np.float64), geom=1, brute=False)}
+    assert mine == ref, (len(mine), len(ref), len(mine ^ ref))

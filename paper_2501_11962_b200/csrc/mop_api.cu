@@ -287,6 +287,14 @@ static mop_status create_impl(mop_ctx **out, const mop_params *p, bool blk, int 
         size_t S = (size_t)c->Q + (size_t)(MOP_CL - 1) * (size_t)g.ncol;
         g.S = (int)((S + 31) / 32 * 32);
     }
+    // what the kernels' index arithmetic assumes: a list entry keeps its j-octet in 24 bits (cj | sid << 24), and the
+    // pair kernels address the sorted arrays with 32-bit element offsets bead * S + slot
+    if (g.S / MOP_CL >= (1 << 24) || (double)c->nf * (double)g.S >= 2147483648.0) {
+        const bool octets = g.S / MOP_CL >= (1 << 24);
+        delete c;
+        return bad(MOP_ERR_INVALID_ARG, octets ? "more than 2^24 atom octets per bead (n_atoms + padding >= 1.34e8)"
+                                               : "force beads * padded slots per bead >= 2^31 (32-bit element offsets)");
+    }
     const size_t nf = c->nf, Q = c->Q, S = g.S;
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) {
@@ -586,9 +594,13 @@ static mop_status build_list_once(mop_ctx *c, const float *R, int nb, bool timed
 
 // the builder keeps counting past the capacities, so an overflowed build tells what a sufficient allocation is
 static mop_status regrow_lists(mop_ctx *c) {
+    // ... but the counts are those of the LAST build only, while the overflow word is sticky across the builds of one call
+    // (the displaced builds of mop_eval_veff_grad_fd, the steps of mop_step): a buffer whose bit is set grows by a factor
+    // even when the last build happened to fit, so that repeating the call cannot meet the same overflow for ever
     const MopCounters &h = *c->h_ctr;
-    const double nu = std::max((double)c->cap_units, 1.05 * h.n_units), ne = std::max((double)c->cap_entries, 1.3 * h.n_entries),
-                 nm = std::max((double)c->cap_masks, 1.3 * h.n_masks);
+    const double gu = (h.overflow & 2u) ? 1.3 : 1.0, ge = (h.overflow & 1u) ? 1.3 : 1.0, gm = (h.overflow & 4u) ? 1.3 : 1.0;
+    const double nu = std::max(gu * (double)c->cap_units, 1.05 * h.n_units), ne = std::max(ge * (double)c->cap_entries, 1.3 * h.n_entries),
+                 nm = std::max(gm * (double)c->cap_masks, 1.3 * h.n_masks);
     if (h.overflow & 24u) FAIL(c, MOP_ERR_OOM, "pair-list builder: per-octet staging (8) or exclusion rows (16) exhausted, flags 0x%x", h.overflow);
     CK(c, cudaStreamSynchronize(c->st));
     mop_status s = alloc_lists(c, nu, ne, nm);
@@ -1289,7 +1301,9 @@ extern "C" mop_status mop_debug_noise_bits(mop_ctx *c, unsigned long long seed, 
 extern "C" mop_status mop_set_bias(mop_ctx *c, const int *group_a, int n_a, const int *group_b, int n_b, double sigma,
                                    double height, int pace) {
     PRECHECK(c);
-    NOT_A_PARTIAL_BLOCK(c);
+    // no block context takes a bias (mop.h), the one that holds the whole path included: mop_block_assemble has no
+    // coordinates to form the CV from, and a sharded path would need the owners of beads 1 and N to exchange s(R)
+    if (c->blk) FAIL(c, MOP_ERR_INVALID_ARG, "mop_set_bias: bead-block contexts take no bias (use mop_create for a biased path)");
     CK(c, cudaStreamSynchronize(c->st));
     c->bias_on = false;
     c->bias_steps = 0;

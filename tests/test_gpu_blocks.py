@@ -85,9 +85,15 @@ def test_block_context_rules_and_integrator(B, oracle):
         a.mop_block_pass1(Rg[:2])
     with pytest.raises(B.MopError):                   # block outside the path
         B.Mop(s, 3, block=(2, 4))
+    with pytest.raises(B.MopError) as e:              # no block context takes a bias (mop.h) ...
+        a.mop_set_bias([0], [1], 0.01, 1.0)
+    assert e.value.status == 1
     a.close()
     # a block that is the whole path takes the whole-path calls
     w = B.Mop(s, 4, block=(0, 4))
+    with pytest.raises(B.MopError) as e:              # ... the one that holds the whole path included: mop_block_assemble
+        w.mop_set_bias([0], [1], 0.01, 1.0)           # has no coordinates to form the CV from
+    assert e.value.status == 1 and "bias" in str(e.value)
     m = B.Mop(s, 4)
     v1, g1 = w.mop_eval_veff_grad(Rg)
     v0, g0 = m.mop_eval_veff_grad(Rg)

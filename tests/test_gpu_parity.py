@@ -766,6 +766,55 @@ def test_pair_list_overflow_is_reported_and_regrown(B, oracle, which):
     m.close()
 
 
+def test_overflow_in_a_middle_build_only_still_grows_the_buffer(B):
+    """The overflow word is sticky across the builds of one call, the builder's counts are those of the LAST build only.
+    Here a dense configuration (all atoms in one octant of the box) overflows the entry buffer and a sparse one (the same
+    atoms spread over the whole box), built right after it without a synchronising call in between, fits with more than
+    the regrow margin to spare.  The flagged buffer must grow all the same, otherwise repeating the sequence meets the
+    same overflow for ever."""
+    s = H.lj_cluster(n=512, L=5.0, seed=4)                            # lattice spacing 0.625 nm: a thin gas
+    rng = np.random.default_rng(11)
+    RB = (s.R1[None] + rng.normal(0, 0.002, (4, s.n_atoms, 3))).astype(np.float32)
+    RA = (0.5 * RB).astype(np.float32)                                # spacing 0.31 nm: 8 x the density, in one octant
+    m = B.Mop(s, 4)
+    vA, gA = m.mop_eval_veff_grad(RA)
+    nA = m.mop_get_stats()["entries"]
+    m.mop_eval_veff_grad(RB)
+    nB = m.mop_get_stats()["entries"]
+    assert nA > 1.45 * nB, (nA, nB)                                   # the premise: 1.3 x the last count is below the capacity
+    m.mop_debug_set_list_capacity(entries=int(1.4 * nB))              # holds RB with > 1.3 x to spare, not RA
+    for attempt in range(8):
+        m.mop_eval_veff_grad(RA, sync=False)                          # overflows (or not any more)
+        m.mop_eval_veff_grad(RB, sync=False)                          # fits; its counts are the ones a regrow sees
+        try:
+            m.mop_get_stats()
+            break
+        except B.MopError as e:
+            assert e.status == 4
+    else:
+        pytest.fail("the entry buffer never grew: the same overflow after 8 repeats (entries %d vs %d)" % (nA, nB))
+    assert attempt >= 1                                               # the first round did overflow
+    v, g = m.mop_eval_veff_grad(RA)                                   # and the dense path now evaluates as it did before
+    assert abs(v - vA) <= 1e-8 * abs(vA) and H.rms_rel(g.cpu().numpy(), gA.cpu().numpy()) <= 1e-6
+    m.close()
+
+
+def test_create_refuses_sizes_beyond_the_index_arithmetic(B):
+    """mop_create checks what the kernels' packed indices assume (24-bit j-octet index in a list entry, 32-bit element
+    offsets bead * S + slot) before it allocates anything."""
+    import ctypes as C
+    L = B.load()
+    for Q, N, box, word in ((140_000_000, 1, (300.0, 300.0, 300.0), b"octets"), (1000, 1_000_000, (1000.0, 1000.0, 2.5), b"2^31")):
+        p = B.mop_params()
+        p.n_atoms, p.n_beads = Q, N
+        p.box[0], p.box[1], p.box[2] = box
+        p.r_cut, p.dt_path, p.nu = 1.0, 0.002, 50.0
+        ctx = C.c_void_p()
+        assert L.mop_create(C.byref(ctx), C.byref(p)) == 1
+        assert word in L.mop_last_error(None), L.mop_last_error(None)
+        assert not ctx.value
+
+
 @pytest.mark.parametrize("bad", [1.0e12, -3.0e30, float("inf"), float("nan")])
 def test_runaway_coordinates_are_reported_not_faulted(B, oracle, bad):
     """A coordinate the wrap cannot bring back into the box (|x| >~ 1e7 L, Inf, NaN) -- what a diverging trajectory

@@ -403,8 +403,9 @@ def test_mop_bias_matches_oracle(B, oracle):
     assert st["V"] == pytest.approx(vb_ref, rel=1e-10)
     dg = (g1 - g0).cpu().numpy().astype(np.float64)
     # interior beads: untouched by the bias; two evaluations differ by the order of the float atomics only (FP32 rounding of
-    # a gradient component, relative to the largest component of that bead block)
-    assert np.abs(dg[1:-1]).max() <= 1e-5 * np.abs(g0[1:-1].cpu().numpy()).max()
+    # a gradient component, relative to the largest component of that bead block).  Measured on a B200: 200 repeated
+    # evaluations of this path, with and without the bias, differ from the first by at most 4.9e-8 max|G|; the bar is 20 x that
+    assert np.abs(dg[1:-1]).max() <= 1e-6 * np.abs(g0[1:-1].cpu().numpy()).max()
     scale = np.abs(gb_ref).max()
     assert np.abs(dg[0] - gb_ref[0]).max() <= 2e-3 * scale and np.abs(dg[-1] - gb_ref[-1]).max() <= 2e-3 * scale
     #   (g1 - g0 is a difference of two FP32 gradients of size ~|G|; the bias part itself is exact to FP32 rounding)

@@ -188,6 +188,21 @@ def workload_name(config, s, beads):
         config - 1, s.name, s.n_atoms, s.box[0], s.box[1], s.box[2], s.r_cut, beads)
 
 
+def bench_config(a, s, N, world, blocks_mode, n_path, temperature, seed):
+    """The `config` object of the JSON line.  Both arms print the same one (the reference arm times the oracle on the GPU
+    arm's config): `workload`, `path` and `pair_list` hold for both; `parallelism` and `l2` describe how the GPU arm runs
+    that workload (the oracle arm runs on the host cores and has no L2 to flush -- its own run is described in its
+    `cpu_baseline.sample`)."""
+    return {"workload": workload_name(a.config, s, N) if not blocks_mode else
+            workload_name(a.config, s, n_path) + " (one path; %d beads per GPU)" % N,
+            "parallelism": "1 GPU" if world == 1 else
+            ("bead blocks: %d ranks x %d beads of one %d-bead path, halos by torch.distributed batch_isend_irecv "
+             "(NCCL point-to-point), V_eff all-reduced (mop.h bead-block mode)" % (world, N, n_path) if blocks_mode
+             else "independent replicas"),
+            "l2": "256 MiB buffer written between timed steps (L2 flush)", "pair_list": "rebuilt every step",
+            "path": "Brownian recursion, dt=2 fs, nu=50/ps, T=%g K, seed %d" % (temperature, seed)}
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(a):
     import torch
@@ -212,7 +227,9 @@ def run_ours(a):
         from paper_2501_11962_b200 import blocks
         n_path = N * world
         first, nb = blocks.partition(n_path, world)[rank]
-        R = W.brownian_path(s, first + nb, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0)[first:]
+        # at most 32 recursion steps, walked back and forth for longer paths: the raw Euler recursion of the stiff water
+        # diverges after ~60 steps, and rank 7 of --gpus 8 would need 63 of them
+        R = W.folded_path(s, first + nb, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0, first=first)
         m1.close()
         m = binding.Mop(s, nb, device=local_rank, block=(first, n_path))
         bp = blocks.BlockPath(m, Q, first, nb, n_path, rank=rank, world=world, device=dev)
@@ -271,6 +288,21 @@ def run_ours(a):
     m.mop_set_timing(False)
     st1 = m.mop_get_stats()
     launches = int(round((st1["launches"] - launches0) / 1.0))
+    # the headline above records stage events, which switches the CUDA-graph replay off; the same K steps with stage
+    # timing off go through the graphs, the form a caller of mop_eval_veff_grad gets (reported beside, not instead)
+    ms_graphs = None
+    if not blocks_mode:
+        eg0 = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps)]
+        eg1 = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps)]
+        for _ in range(2):
+            step()
+        for k in range(a.steps):
+            flush.zero_()
+            eg0[k].record()
+            step()
+            eg1[k].record()
+        torch.cuda.synchronize()
+        ms_graphs = float(sum(eg0[k].elapsed_time(eg1[k]) for k in range(a.steps))) / a.steps
     ms_max, units = all_reduce_max_sum(local_ms, float(Rd.shape[0] * a.steps), world, dev)
     if world > 1:   # pair counts of all ranks (rank 0 reports the job's pair rate; the roofline stays rank 0's own kernel)
         pc = torch.tensor([pairs_force, pairs_hvp], dtype=torch.float64, device=dev)
@@ -355,13 +387,8 @@ def run_ours(a):
         "metric": METRIC, "value": throughput(units, ms_max), "unit": UNIT, "n_gpus": world, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(a.config, s, N) if not blocks_mode else
-                   workload_name(a.config, s, n_path) + " (one path; %d beads per GPU)" % N,
-                   "parallelism": "1 GPU" if world == 1 else
-                   ("bead blocks: %d ranks x %d beads of one %d-bead path, halos by NCCL send/recv, V_eff all-reduced "
-                    "(mop.h bead-block mode)" % (world, N, n_path) if blocks_mode else "independent replicas"),
-                   "l2": "256 MiB buffer written between timed steps (L2 flush)", "pair_list": "rebuilt every step",
-                   "path": "Brownian recursion, dt=2 fs, nu=50/ps, T=%g K, seed %d" % (s.temperature, rank)},
+        "config": bench_config(a, s, N, world, blocks_mode, n_path, s.temperature, rank),
+        "ms_per_step_graphs": ms_graphs,
         "pair_interactions_per_sec": (pairs_force_job + pairs_hvp_job) / (ms_per_step * 1e-3),
         "pairs_in_range_per_bead": pairs_force / max(m.nf, 1),
         "pair_slots_admitted_by_patterns_per_pass": st1["pair_slots"],
@@ -412,8 +439,11 @@ def cpu_baseline(s, N):
     out = {"value": N * (nfb / float(nf)) / dt_all, "unit": UNIT, "cores": min(threads, nfb), "kind": "oracle",
            "sample": "one whole V_eff-gradient evaluation of the first %d beads of the workload path on the full %d-atom "
                      "system (%d force beads: force pass + H.eta pass each, %d in-range pairs in total), %.1f s on %d of "
-                     "%d available threads%s" % (nb, s.n_atoms, nfb, parts["npairs"], dt_all, min(threads, nfb), threads,
-                                                 "" if nb == N else "; scaled to %d force beads" % nf),
+                     "%d available threads%s; the path comes from the same recursion and seed as the GPU arm's but with the "
+                     "oracle's FP64 force in it (the GPU arm's uses the library's pass 1), so the two arms time equal "
+                     "workloads, not byte-identical inputs"
+                     % (nb, s.n_atoms, nfb, parts["npairs"], dt_all, min(threads, nfb), threads,
+                        "" if nb == N else "; scaled to %d force beads" % nf),
            "seconds": dt_all, "pair_interactions_per_sec": 2.0 * parts["npairs"] / dt_all}
     if nb >= 2:
         t = time.perf_counter()
@@ -466,7 +496,7 @@ def run_reference(a):
     return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world, "steps": done,
             "warmup": warm_done, "ms_per_step": dt * 1e3 / done, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(a.config, s, N)},
+            "config": bench_config(a, s, N, world, a.parallelism == "blocks" and world > 1, N * world, s.temperature, 0),
             "pair_interactions_per_sec": 2.0 * parts["npairs"] * done / dt,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": min(threads, nf), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},

@@ -248,7 +248,7 @@ mop_status mop_debug_set_list_capacity(mop_ctx *c, unsigned units, unsigned entr
  *   from the right neighbour, before pass 1: R_right = its first bead R^{n1} (eta of the block's last bead);
  *   from the left neighbour, before the assembly: K eta^{n0-1}, which that neighbour's mop_block_pass1 writes to its
  *     keta_right_out_dev (the spring term K eta^{n-1} of eqs (5),(7)).
- * The library does no communication: the caller moves the halos (bench.py: torch.distributed send/recv over NCCL) and sums
+ * The library does no communication: the caller moves the halos (blocks.py: torch.distributed batch_isend_irecv, NCCL point-to-point) and sums
  * the per-block V_eff values (an 8-byte all-reduce).  Call order per evaluation: mop_block_pass1 (S0-S4), mop_block_pass2
  * (S5-S6), mop_block_assemble (S7); the halo for the right neighbour is ready once pass1 has run, so its transfer overlaps
  * pass 2.  Force, eta and H.eta run on every bead of the block except the path's last bead; U(R^1) only in the block with

@@ -29,13 +29,9 @@ def run(config, N, steps, pmd_steps, device=0, r_buf=0.0):
     dev = torch.device("cuda", device)
     s = W.CONFIGS[config](seed=0, n_beads=N)
     m1 = binding.Mop(s, 1, device=device)
-    L = min(N, 32)
-    R = W.brownian_path(s, L, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0)
+    # N > 32: back and forth over the stable stretch of the recursion (workloads.folded_path)
+    R = W.folded_path(s, N, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0)
     m1.close()
-    if N > L:   # back and forth over the stable stretch of the recursion
-        idx = [j % (2 * (L - 1)) for j in range(N)]
-        idx = [j if j < L else 2 * (L - 1) - j for j in idx]
-        R = np.ascontiguousarray(R[idx])
     m = binding.Mop(s, N, device=device)
     Rd = torch.as_tensor(R, device=dev)
     Gd = torch.empty_like(Rd)

@@ -4,6 +4,9 @@ water-like box with N = 64 beads; the paper's own run is 512 beads x ~150k atoms
 
     python -m paper_2501_11962_b200.validate [--config 2] [--beads 64] [--steps 2000] [--dt 0.0005]
 
+At the paper's PMD step (--dt 0.001) the Lennard-Jones config 1 runs (profiles/r03_validate_fig4.txt); the
+unconstrained water stand-in of config 2 needs 0.5 fs, the default here (the paper constrains bonds to H, out of scope).
+
 Prints one JSON line per ensemble.  NVE: velocity Verlet (mop_step) from thermal velocities; reports the standard
 deviation and the drift of V_eff + E_kin relative to the mean kinetic energy.  NVT: mop_step_langevin with the paper's
 damping (250 /ps) from rest; reports mean and standard deviation of the kinetic temperature after

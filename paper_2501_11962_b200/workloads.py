@@ -438,6 +438,25 @@ def brownian_path(system, n_beads, force_fn, seed=0, noise=True, dtype=np.float3
     return R.astype(dtype)
 
 
+MAX_RECURSION_BEADS = 32
+
+
+def folded_path(system, n_beads, force_fn, seed=0, noise=True, dtype=np.float32, first=0):
+    """Beads [first, n_beads) of a path of any length from at most MAX_RECURSION_BEADS steps of the Brownian recursion.
+
+    The explicit Euler recursion of the stiff three-site water is only stable for a few dozen steps,
+    so a longer path walks the stable stretch back and forth: bead j is recursion bead j mod 2(L-1), reflected at L-1.
+    Neighbouring beads stay one recursion step apart, which is all eqs (3),(5)-(7) look at.  For n_beads <= 32 this is
+    brownian_path itself."""
+    L = min(n_beads, MAX_RECURSION_BEADS)
+    R = brownian_path(system, L, force_fn, seed=seed, noise=noise, dtype=dtype)
+    if n_beads <= L and first == 0:
+        return R
+    idx = [j % (2 * (L - 1)) if L > 1 else 0 for j in range(first, n_beads)]
+    idx = [j if j < L else 2 * (L - 1) - j for j in idx]
+    return np.ascontiguousarray(R[idx])
+
+
 def min_nonexcluded_distance(system, X, r_probe=0.25):
     """Smallest periodic distance between non-excluded atoms (generator sanity gate)."""
     box = np.asarray(system.box, float)

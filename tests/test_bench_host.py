@@ -61,3 +61,45 @@ def test_roofline_traffic_comes_from_the_committed_ncu_capture():
     vals = dict(l.strip().split(",") for l in open(os.path.join(ROOT, src)) if not l.startswith("#"))
     assert traffic == float(vals["dram__bytes_read.sum"]) + float(vals["dram__bytes_write.sum"])
     assert 1.0e7 < traffic < 1.0e10          # bytes per launch: tens to hundreds of MB
+
+
+def test_both_arms_print_the_same_config_object():
+    """The reference arm times the oracle on the GPU arm's `config`: one function builds it for both (the driver compares
+    the two dicts key by key)."""
+    sys.path.insert(0, ROOT)
+    import argparse
+    import bench
+    from paper_2501_11962_b200 import workloads as W
+    s = W.config1(n_beads=16)
+    a = argparse.Namespace(config=1, parallelism="blocks")
+    c = bench.bench_config(a, s, 16, 1, False, 16, s.temperature, 0)
+    assert sorted(c) == ["l2", "pair_list", "parallelism", "path", "workload"]
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": bench_config(') == 2          # run_ours and run_reference
+
+
+def test_folded_path_is_the_recursion_walked_back_and_forth():
+    """workloads.folded_path (bench.py --gpus N, sweep.py): at most 32 recursion steps whatever the path length; every pair
+    of neighbouring beads is one recursion step apart; a rank's slice equals the same beads of the whole path."""
+    import numpy as np
+    from paper_2501_11962_b200 import workloads as W
+    s = W.config1(n_beads=16)
+    calls = []
+
+    def zero_force(X):
+        calls.append(1)
+        return np.zeros_like(X)
+
+    R16 = W.folded_path(s, 16, zero_force, seed=3)
+    assert np.array_equal(R16, W.brownian_path(s, 16, zero_force, seed=3))
+    del calls[:]
+    R70 = W.folded_path(s, 70, zero_force, seed=3)
+    assert len(calls) == W.MAX_RECURSION_BEADS - 1 and R70.shape == (70, s.n_atoms, 3)
+    R32 = W.brownian_path(s, 32, zero_force, seed=3)
+    assert np.array_equal(R70[:32], R32) and np.array_equal(R70[32], R32[30]) and np.array_equal(R70[62], R32[0])
+    assert np.array_equal(R70[63], R32[1])
+    steps = {tuple(sorted((int(np.argmin([np.abs(R32[k] - R70[j]).max() for k in range(32)])),
+                           int(np.argmin([np.abs(R32[k] - R70[j + 1]).max() for k in range(32)]))))) for j in range(69)}
+    assert all(b - a == 1 for a, b in steps)
+    assert np.array_equal(W.folded_path(s, 70, zero_force, seed=3, first=56), R70[56:])
+    assert W.folded_path(s, 1, zero_force, seed=3).shape == (1, s.n_atoms, 3)

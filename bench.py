@@ -246,7 +246,7 @@ def run_ours(a):
 
     def step():
         if blocks_mode:
-            bp.eval(Rd, grad_out=Gd)        # halos over NCCL, V_eff all-reduced (the host reads 8 bytes per step)
+            bp.eval(Rd, grad_out=Gd, sync=False)   # halos over NCCL; like the whole-path arm, no V_eff read per step
         else:
             m.mop_eval_veff_grad(Rd, sync=False, grad_out=Gd)
 
@@ -287,6 +287,7 @@ def run_ours(a):
     stages = m.mop_get_timing()
     m.mop_set_timing(False)
     st1 = m.mop_get_stats()
+    veff_job = bp.veff() if blocks_mode else st1["veff"]    # whole-path V_eff (blocks: one 8-byte all-reduce, all ranks)
     launches = int(round((st1["launches"] - launches0) / 1.0))
     # the headline above records stage events, which switches the CUDA-graph replay off; the same K steps with stage
     # timing off go through the graphs, the form a caller of mop_eval_veff_grad gets (reported beside, not instead)
@@ -381,7 +382,6 @@ def run_ours(a):
     ach = pairs_hvp * FLOP_PER_PAIR_HVP / t_hvp / 1e12 if t_hvp > 0 else 0.0
     ach_f = pairs_force * FLOP_PER_PAIR_FORCE / t_force / 1e12 if t_force > 0 else 0.0
     ms_per_step = ms_max / a.steps
-    probe = binding.mop_probe_fp32(local_rank)   # dependent-free FMA streams (context for the nominal peak, not a denominator)
     traffic, traffic_src = traffic_bytes_per_launch()
     out = {
         "metric": METRIC, "value": throughput(units, ms_max), "unit": UNIT, "n_gpus": world, "steps": a.steps,
@@ -401,7 +401,6 @@ def run_ours(a):
                      "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz, %s MEASURED_PEAKS.json); "
                                     "no measured FP32 entry exists" % (sm_max, peak_src),
                      "flop_per_pair": FLOP_PER_PAIR_HVP, "pairs_per_launch": pairs_hvp, "ms_per_launch": stages["S5_nb_hvp"],
-                     "fp32_probe_tflops": {k: round(v, 2) for k, v in probe.items() if k != "sms"},
                      "force_kernel": {"achieved": ach_f, "frac": ach_f / peak_tf, "flop_per_pair": FLOP_PER_PAIR_FORCE,
                                       "pairs_per_launch": pairs_force, "ms_per_launch": stages["S2_nb_force"]}},
         "e2e": {"value": throughput(e2e_units, e2e_ms_max), "unit": UNIT, "h2d_bytes_per_step": int(n_path) * Q * 12,
@@ -411,7 +410,7 @@ def run_ours(a):
         "with_list_reuse": reuse,
         "gpu_launches": launches,
         "clocks": clk,
-        "veff": st1["veff"],
+        "veff": veff_job,
     }
     if world == 1 and not a.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(s, N)

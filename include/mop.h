@@ -254,7 +254,8 @@ mop_status mop_debug_set_list_capacity(mop_ctx *c, unsigned units, unsigned entr
  * pass 2.  Force, eta and H.eta run on every bead of the block except the path's last bead; U(R^1) only in the block with
  * first_bead = 0.  A block that is the whole path (first_bead = 0, n_beads = n_beads_path) also accepts the whole-path calls
  * above; other block contexts refuse them (INVALID_ARG), and none of them takes a bias.  The sum over blocks of
- * veff_local_out is V_eff; the blocks' gradients are the rows of the whole-path gradient.
+ * veff_local_out is V_eff; the blocks' gradients are the rows of the whole-path gradient.  Path MD on a sharded path: every
+ * bead moves with its own gradient, so mop_block_integrate (NVE) and mop_block_thermostat (NVT) need no exchange.
  * Errors: as mop_create / mop_eval_veff_grad; INVALID_ARG for a block outside the path, a missing halo, or calls out of order. */
 mop_status mop_create_block(mop_ctx **out, const mop_params *p, int first_bead, int n_beads_path);
 mop_status mop_block_pass1(mop_ctx *c, const float *R_dev, const float *R_right_dev, float *keta_right_out_dev);
@@ -266,6 +267,16 @@ mop_status mop_block_assemble(mop_ctx *c, const float *keta_left_dev, double *ve
  * with its own gradient, so the integrator needs no exchange): stage 0: v += dt/2 (-grad)/m; R += dt v.  stage 1:
  * v += dt/2 (-grad)/m.  Works on any context. */
 mop_status mop_block_integrate(mop_ctx *c, float *R_dev, float *V_dev, const float *grad_dev, double dt_pmd, int stage);
+/* The thermostat half of an NVT step on the block's beads -- the configuration of the paper's scaling runs ("for each polymer
+ * size, we have performed an NVT simulation"; Langevin, damping 0.25 fs^-1): the exact
+ * Ornstein-Uhlenbeck update of mop_step_langevin (reading G19), v <- c v + sqrt((1 - c^2) k_B T / m_i) xi, applied to
+ * V_dev DEVICE [n_beads][Q][3] after stage 1 of mop_block_integrate.  The generator is keyed by (seed, step, index of the
+ * coordinate in the WHOLE path's [n_beads_path][Q][3] array), so the blocks of a sharded run together draw exactly the numbers
+ * one mop_step_langevin call on the whole path draws for PMD step `step` (= its step0 + step index): no exchange is needed
+ * and the trajectory does not depend on how the path is cut.  gamma = 0 does nothing.  Works on any context (first bead 0
+ * for a whole-path context).  Asynchronous.  Errors: INVALID_ARG. */
+mop_status mop_block_thermostat(mop_ctx *c, float *V_dev, double dt_pmd, double gamma, double temperature,
+                                unsigned long long seed, unsigned long long step);
 
 /* ---- for callers that must not allocate device memory ------------------------------------------------------------------
  * Everything above works on a context, and a context allocates (mop_create, mop_set_topology, list regrowth).  Some callers

@@ -21,7 +21,7 @@ EXPORTS = ["mop_create", "mop_set_topology", "mop_eval_veff_grad", "mop_step", "
            "mop_step_langevin_continue", "mop_debug_count_inrange", "mop_create_block", "mop_block_pass1",
            "mop_block_pass2", "mop_block_assemble", "mop_block_integrate", "mop_debug_set_list_capacity",
            "mop_step_langevin", "mop_debug_noise_bits", "mop_set_bias", "mop_add_hill", "mop_get_bias",
-           "mop_eta_spring_noalloc"]
+           "mop_eta_spring_noalloc", "mop_block_thermostat"]
 MOP_NOALLOC_MAX_ATOM_BEADS = 33554432   # include/mop.h
 
 
@@ -51,17 +51,23 @@ def lib_path():
     return _build.LIB
 
 
-def load(build_if_missing=True):
-    """Loads the C-ABI library (building it with nvcc when it is missing or stale).  Raises if unavailable."""
+def load(build_if_missing=True, path=None):
+    """Loads the C-ABI library (building it with nvcc when it is missing or stale).  Raises if unavailable.
+    path: load that build of the library instead (first call of the process only; the -DMOP_CHECK build of
+    tests/sanitizer_target.py --checked)."""
     global _lib
     if _lib is not None:
+        if path is not None:
+            raise RuntimeError("the library is already loaded")
         return _lib
-    if build_if_missing:
-        _build.build()
-    if not os.path.exists(_build.LIB):
-        raise RuntimeError("libmop_b200.so is not built (run python -m paper_2501_11962_b200.build); "
-                           "there is no CPU fallback")
-    L = C.CDLL(_build.LIB)
+    if path is None:
+        if build_if_missing:
+            _build.build()
+        path = _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError("%s is not built (run python -m paper_2501_11962_b200.build); there is no CPU fallback"
+                           % os.path.basename(path))
+    L = C.CDLL(path)
     L.mop_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(mop_params)]
     L.mop_set_topology.argtypes = [C.c_void_p, C.POINTER(mop_topology)]
     L.mop_eval_veff_grad.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.c_void_p]
@@ -93,6 +99,8 @@ def load(build_if_missing=True):
     L.mop_block_assemble.restype = C.c_int
     L.mop_block_integrate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int]
     L.mop_block_integrate.restype = C.c_int
+    L.mop_block_thermostat.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64]
+    L.mop_block_thermostat.restype = C.c_int
     L.mop_eval_veff_grad_fd.argtypes = [C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.c_void_p]
     L.mop_eval_veff_grad_fd.restype = C.c_int
     L.mop_step_langevin.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_double,
@@ -116,20 +124,6 @@ def load(build_if_missing=True):
         getattr(L, n).restype = C.c_int
     _lib = L
     return L
-
-
-def mop_probe_fp32(device=0):
-    """Achieved TFLOP/s of dependent-free FMA streams: reused-operand FFMA, three-register FFMA, three-register-pair
-    FFMA2.  A measurement aid for bench.py; it lives in its own small library (csrc/mop_probe.cu), not in the product."""
-    _build.build()
-    P = C.CDLL(_build.PROBE_LIB)
-    P.mop_probe_fp32.argtypes = [C.c_int, C.POINTER(C.c_double)]
-    P.mop_probe_fp32.restype = C.c_int
-    out = (C.c_double * 4)()
-    st = P.mop_probe_fp32(int(device), out)
-    if st != 0:
-        raise MopError(st, "mop_probe_fp32 failed")
-    return {"ffma_reuse_tflops": out[0], "ffma_3reg_tflops": out[1], "ffma2_3reg_tflops": out[2], "sms": int(out[3])}
 
 
 def _ptr(t):
@@ -332,6 +326,12 @@ class Mop:
     def mop_block_integrate(self, R, V, grad, dt_pmd, stage):
         assert R.is_cuda and V.is_cuda and grad.is_cuda and R.shape == V.shape == grad.shape
         self._check(self.L.mop_block_integrate(self.ctx, _ptr(R), _ptr(V), _ptr(grad), float(dt_pmd), int(stage)))
+
+    def mop_block_thermostat(self, V, dt_pmd, gamma, temperature, seed=0, step=0):
+        """The OU velocity update of mop_step_langevin on this context's beads, noise keyed by the whole-path index."""
+        assert V.is_cuda and V.is_contiguous() and tuple(V.shape) == (self.N, self.Q, 3)
+        self._check(self.L.mop_block_thermostat(self.ctx, _ptr(V), float(dt_pmd), float(gamma), float(temperature), int(seed),
+                                                int(step)))
 
     def mop_set_bias(self, group_a, group_b, sigma, height, pace=0):
         """MoP bias on S_e2e = s(R^N) - s(R^1), s = COM distance of the two groups.  Empty groups switch it off."""

@@ -66,8 +66,10 @@ class BlockPath:
         self.R_right, self.keta_out, self.keta_left = mk(), mk(), mk()
         self._vbuf = torch.zeros(1, dtype=torch.float64, device=device)
 
-    def eval(self, R_block, grad_out=None):
-        """R_block [n_beads][Q][3] (this rank's beads).  Returns (V_eff of the WHOLE path, gradient of this block)."""
+    def eval(self, R_block, grad_out=None, sync=True):
+        """R_block [n_beads][Q][3] (this rank's beads).  Returns (V_eff of the WHOLE path, gradient of this block).
+        sync=False: the assembly stays asynchronous and no V_eff is formed (returns (None, gradient)): a stepping loop needs
+        the gradient only; read the energy when it is wanted with veff()."""
         # 1. right halo of the coordinates
         _wait(_exchange(self.left, R_block[0].contiguous(), self.right, self.R_right, self.group))
         # 2. pass 1
@@ -79,9 +81,18 @@ class BlockPath:
         self.engine.mop_block_pass2(R_block)
         _wait(reqs)
         # 5. assembly and the 8-byte reduction
+        if not sync:
+            return self.engine.mop_block_assemble(self.keta_left if self.has_left else None, grad_out, sync=False)
         v_local, grad = self.engine.mop_block_assemble(self.keta_left if self.has_left else None, grad_out)
+        return self._reduce(v_local), grad
+
+    def veff(self):
+        """V_eff of the whole path at the last evaluation (synchronises this rank's stream; 8-byte all-reduce)."""
+        return self._reduce(self.engine.mop_get_stats()["veff"])
+
+    def _reduce(self, v_local):
         if self.world > 1:
             self._vbuf[0] = v_local
             dist.all_reduce(self._vbuf, op=dist.ReduceOp.SUM, group=self.group)
             v_local = float(self._vbuf.item())
-        return v_local, grad
+        return v_local

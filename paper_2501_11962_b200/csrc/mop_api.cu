@@ -1172,6 +1172,24 @@ extern "C" mop_status mop_block_integrate(mop_ctx *c, float *R_dev, float *V_dev
     return MOP_OK;
 }
 
+// the thermostat half of an NVT step on a bead block: the OU update of mop_step_langevin with the generator keyed by the
+// coordinate's index in the whole path, so that every rank of a sharded run replays its part of the one noise stream
+extern "C" mop_status mop_block_thermostat(mop_ctx *c, float *V_dev, double dt_pmd, double gamma, double temperature,
+                                           unsigned long long seed, unsigned long long step) {
+    PRECHECK(c);
+    if (!V_dev) FAIL(c, MOP_ERR_INVALID_ARG, "V_dev is NULL");
+    if (!(dt_pmd > 0.0) || !(gamma >= 0.0) || !(temperature >= 0.0)) FAIL(c, MOP_ERR_INVALID_ARG, "need dt_pmd > 0, gamma >= 0 and temperature >= 0");
+    if (gamma == 0.0) return MOP_OK;   // plain velocity Verlet
+    const double cc = exp(-gamma * dt_pmd);
+    const float amp = (float)sqrt((1.0 - cc * cc) * 0.0083144626 * temperature);   // k_B in kJ mol^-1 K^-1
+    const size_t total = (size_t)c->N * c->Q * 3;
+    const unsigned long long idx0 = (unsigned long long)(c->blk ? c->blk_n0 : 0) * (unsigned long long)c->Q * 3ull;
+    LAUNCH(c, k_ou, cdiv(total, 256), 256, 0, total, c->Q, (float)cc, amp, seed, step, idx0, c->d_inv_mass, c->d_mass, V_dev,
+           (double *)nullptr);
+    CK(c, cudaGetLastError());
+    return MOP_OK;
+}
+
 extern "C" mop_status mop_set_timing(mop_ctx *c, int on) {
     if (!c) return MOP_ERR_INVALID_ARG;
     if (c->sticky) return (mop_status)c->sticky;
@@ -1240,7 +1258,7 @@ static mop_status step_impl(mop_ctx *c, float *R_dev, float *V_dev, double dt_pm
         LAUNCH(c, k_verlet, nblk, 256, 0, total, c->Q, (float)dt_pmd, 1, c->d_inv_mass, c->d_mass, c->d_G, R_dev, V_dev,
                (last && !ou) ? c->d_energy + 5 : (double *)nullptr);
         if (ou)
-            LAUNCH(c, k_ou, nblk, 256, 0, total, c->Q, (float)cc, amp, seed, step0 + (unsigned long long)it, c->d_inv_mass,
+            LAUNCH(c, k_ou, nblk, 256, 0, total, c->Q, (float)cc, amp, seed, step0 + (unsigned long long)it, 0ull, c->d_inv_mass,
                    c->d_mass, V_dev, last ? c->d_energy + 5 : (double *)nullptr);
     }
     CK(c, cudaGetLastError());

@@ -192,15 +192,17 @@ __device__ __forceinline__ float mop_noise_normal(unsigned long long seed, unsig
 }
 
 // exact Ornstein-Uhlenbeck velocity update over dt: v <- c v + sqrt((1 - c^2) kT / m) xi  (+ kinetic energy)
+// idx0: index of V[0] in the whole path's [N][Q][3] array (0 unless V is a bead block of a longer path: the generator is
+// keyed by the coordinate's place in the WHOLE path, so a sharded run draws the numbers the unsharded one does)
 __global__ void __launch_bounds__(256) k_ou(size_t total, int Q, float c, float amp, unsigned long long seed,
-                                            unsigned long long step, const float *__restrict__ inv_m,
+                                            unsigned long long step, unsigned long long idx0, const float *__restrict__ inv_m,
                                             const float *__restrict__ m, float *__restrict__ V,
                                             double *__restrict__ e_kin) {
     const size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     double ek = 0.0;
     if (o < total) {
         const int i = (int)((o / 3) % (size_t)Q);
-        const float v = fmaf(c, V[o], amp * sqrtf(inv_m[i]) * mop_noise_normal(seed, step, o));
+        const float v = fmaf(c, V[o], amp * sqrtf(inv_m[i]) * mop_noise_normal(seed, step, idx0 + o));
         V[o] = v;
         if (e_kin) ek = 0.5 * (double)m[i] * (double)v * (double)v;
     }

@@ -2,8 +2,9 @@
 
     compute-sanitizer --tool memcheck  python tests/sanitizer_target.py
     compute-sanitizer --tool racecheck python tests/sanitizer_target.py
-    python tests/sanitizer_target.py --checked      (where compute-sanitizer is not available: rebuilds the library with
-                                                     -DMOP_CHECK, device-side bounds assertions, runs, rebuilds it plain)
+    python tests/sanitizer_target.py --checked      (where compute-sanitizer is not available: builds the library with
+                                                     -DMOP_CHECK, device-side bounds assertions, as libmop_b200_checked.so
+                                                     and runs the tour on that; tests/test_gpu_checked_build.py does this)
 
 on a B200 (one tool per gpurun call).  Small systems only -- the sanitizer slows kernels by two orders of magnitude:
 __graft_entry__.smoke(), then config 1 (512 LJ atoms, N = 16) through the device and host entry points, mop_step with a
@@ -20,15 +21,11 @@ sys.path.insert(0, ROOT)
 
 def main():
     checked = "--checked" in sys.argv
-    if checked:   # the library with -DMOP_CHECK: device-side bounds assertions on every index derived from list data
-        from paper_2501_11962_b200 import build
-        build.build(force=True, extra=["-DMOP_CHECK"])
-    try:
-        tour()
-    finally:
-        if checked:
-            from paper_2501_11962_b200 import build
-            build.build(force=True)
+    if checked:   # the library with -DMOP_CHECK: device-side bounds assertions on every index derived from list data,
+        # built under its own file name and loaded instead of the product library, which is not touched
+        from paper_2501_11962_b200 import binding, build
+        binding.load(path=build.build(extra=["-DMOP_CHECK"], out=build.CHECKED_LIB))
+    tour()
     print("checked build (-DMOP_CHECK): no assertion fired" if checked else "plain build")
 
 

@@ -33,7 +33,9 @@ class ToyEngine:
             keta_out.copy_(K * self.eta[self.nh - 1])
     def mop_block_pass2(self, R):
         pass
-    def mop_block_assemble(self, keta_left, grad_out):
+    def mop_get_stats(self):
+        return {"veff": self.v}
+    def mop_block_assemble(self, keta_left, grad_out, sync=True):
         g = torch.zeros_like(self.R)
         g[:self.nh] -= K * self.eta
         g[1:self.nh + 1 if self.nh < self.n else self.n] += K * self.eta[:self.n - 1]
@@ -43,7 +45,8 @@ class ToyEngine:
         if self.first == 0:
             g[0] += KW * self.R[0]
             v += 0.5 * KW * float((self.R[0] ** 2).sum())
-        return v, g
+        self.v = v
+        return (v if sync else None), g
 
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
@@ -60,7 +63,10 @@ G[1:] += K * d
 G[0] += KW * R[0]
 V = 0.5 * K * float((d ** 2).sum()) + 0.5 * KW * float((R[0] ** 2).sum())
 err = float((g - G[first:first + n]).abs().max())
-out = torch.tensor([err, abs(v - V)], dtype=torch.float64)
+# the stepping form: no V_eff per evaluation (the assembly stays asynchronous), the energy read once afterwards
+v2, g2 = bp.eval(R[first:first + n].clone(), sync=False)
+assert v2 is None and float((g2 - g).abs().max()) == 0.0
+out = torch.tensor([err, max(abs(v - V), abs(bp.veff() - V))], dtype=torch.float64)
 dist.all_reduce(out, op=dist.ReduceOp.MAX)
 if rank == 0:
     print(json.dumps({"grad_err": float(out[0]), "veff_err": float(out[1]), "world": world, "V": V}))

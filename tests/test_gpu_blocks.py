@@ -115,6 +115,57 @@ def test_block_context_rules_and_integrator(B, oracle):
     m.close()
 
 
+@pytest.mark.parametrize("parts", [[(0, 2), (2, 2)], [(0, 1), (1, 2), (3, 1)]])
+def test_sharded_langevin_step_replays_the_whole_path_noise(B, oracle, parts):
+    """NVT on a sharded path (the configuration of the paper's scaling runs): block evaluation + the two
+    mop_block_integrate halves + mop_block_thermostat per block reproduce mop_step_langevin on the whole path, velocities
+    to 1e-5 RMS -- which they can only do if every block draws, for each of its coordinates, the random number the whole-path
+    call draws (the thermostat term is the larger part of the velocity here: c = exp(-0.25) = 0.78)."""
+    import torch
+    s = W.config1(n_beads=4)
+    o = oracle.OracleSystem(s)
+    R = W.brownian_path(s, 4, lambda X: oracle.bead(o, X, geom=0)["F"], seed=0)
+    rng = np.random.default_rng(3)
+    sd = np.sqrt(W.KB * s.temperature / s.mass.astype(np.float64))
+    V0 = (rng.normal(0, 1, R.shape) * sd[None, :, None]).astype(np.float32)
+    dt, gamma, T, seed, step0 = 0.001, 250.0, s.temperature, 17, 5
+    m = B.Mop(s, 4)
+    Ra, Va = torch.tensor(R, device="cuda"), torch.tensor(V0, device="cuda")
+    m.mop_step_langevin(Ra, Va, dt, 2, gamma, T, seed=seed, step0=step0)
+    m.close()
+    ctx = [B.Mop(s, n, block=(f, 4)) for f, n in parts]
+    Rb = [torch.tensor(R[f:f + n], device="cuda") for f, n in parts]
+    Vb = [torch.tensor(V0[f:f + n], device="cuda") for f, n in parts]
+    keta = [torch.zeros((s.n_atoms, 3), device="cuda") for _ in parts]
+
+    def grads():
+        for k, (f, n) in enumerate(parts):
+            last = f + n == 4
+            ctx[k].mop_block_pass1(Rb[k], None if last else Rb[k + 1][0].contiguous(), None if last else keta[k])
+        for k in range(len(parts)):
+            ctx[k].mop_block_pass2(Rb[k])
+        return [ctx[k].mop_block_assemble(None if k == 0 else keta[k - 1])[1] for k in range(len(parts))]
+
+    g = grads()
+    for it in range(2):
+        for k in range(len(parts)):
+            ctx[k].mop_block_integrate(Rb[k], Vb[k], g[k], dt, 0)
+        g = grads()
+        for k in range(len(parts)):
+            ctx[k].mop_block_integrate(Rb[k], Vb[k], g[k], dt, 1)
+            ctx[k].mop_block_thermostat(Vb[k], dt, gamma, T, seed=seed, step=step0 + it)
+    Vs = torch.cat(Vb).cpu().numpy()
+    Rs = torch.cat(Rb).cpu().numpy()
+    assert H.rms_rel(Vs, Va.cpu().numpy()) <= 1e-5
+    assert H.rms_rel(Rs - R, Ra.cpu().numpy() - R) <= 1e-5
+    # a block that used its LOCAL coordinate index would draw bead 1's numbers again: the velocities would be far apart
+    assert H.rms_rel(Vs[2:], Va.cpu().numpy()[:2]) > 0.1
+    with pytest.raises(B.MopError):
+        ctx[0].mop_block_thermostat(Vb[0], dt, -1.0, T)
+    for c in ctx:
+        c.close()
+
+
 def test_block_path_driver_single_rank(B, oracle):
     """blocks.BlockPath with world = 1 (no process group): the driver bench.py uses, on the real engine."""
     import torch

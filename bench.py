@@ -197,7 +197,9 @@ def bench_config(a, s, N, world, blocks_mode, n_path, temperature, seed):
             workload_name(a.config, s, n_path) + " (one path; %d beads per GPU)" % N,
             "parallelism": "1 GPU" if world == 1 else
             ("bead blocks: %d ranks x %d beads of one %d-bead path, halos by torch.distributed batch_isend_irecv "
-             "(NCCL point-to-point), V_eff all-reduced (mop.h bead-block mode)" % (world, N, n_path) if blocks_mode
+             "(%s), V_eff all-reduced (mop.h bead-block mode)"
+             % (world, N, n_path, "gloo through host memory, ALL RANKS ON ONE GPU: functional run, not a scaling number"
+                if getattr(a, "all_ranks_on_one_gpu", False) else "NCCL point-to-point") if blocks_mode
              else "independent replicas"),
             "l2": "256 MiB buffer written between timed steps (L2 flush)", "pair_list": "rebuilt every step",
             "path": "Brownian recursion, dt=2 fs, nu=50/ps, T=%g K, seed %d" % (temperature, seed)}
@@ -210,11 +212,18 @@ def run_ours(a):
     rank, local_rank, world = env_rank()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the MoP hot path has no CPU fallback")
+    if a.all_ranks_on_one_gpu:      # functional run of the N-rank code path on a single GPU (not a scaling number)
+        local_rank = 0
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    gloo = a.dist_backend == "gloo"
+    rdev = None if gloo else dev    # where the small reduction tensors live
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+        if gloo:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=dev)
     binding.load()
     N = a.beads
     s = build_system(a.config, N)
@@ -232,7 +241,7 @@ def run_ours(a):
         R = W.folded_path(s, first + nb, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0, first=first)
         m1.close()
         m = binding.Mop(s, nb, device=local_rank, block=(first, n_path))
-        bp = blocks.BlockPath(m, Q, first, nb, n_path, rank=rank, world=world, device=dev)
+        bp = blocks.BlockPath(m, Q, first, nb, n_path, rank=rank, world=world, device=dev, host_staging=gloo)
         n_hvp_local = min(nb, n_path - 1 - first)
     else:
         n_path = N
@@ -304,9 +313,9 @@ def run_ours(a):
             eg1[k].record()
         torch.cuda.synchronize()
         ms_graphs = float(sum(eg0[k].elapsed_time(eg1[k]) for k in range(a.steps))) / a.steps
-    ms_max, units = all_reduce_max_sum(local_ms, float(Rd.shape[0] * a.steps), world, dev)
+    ms_max, units = all_reduce_max_sum(local_ms, float(Rd.shape[0] * a.steps), world, rdev)
     if world > 1:   # pair counts of all ranks (rank 0 reports the job's pair rate; the roofline stays rank 0's own kernel)
-        pc = torch.tensor([pairs_force, pairs_hvp], dtype=torch.float64, device=dev)
+        pc = torch.tensor([pairs_force, pairs_hvp], dtype=torch.float64, device=rdev)
         torch.distributed.all_reduce(pc)
         pairs_force_job, pairs_hvp_job = float(pc[0]), float(pc[1])
     else:
@@ -365,7 +374,7 @@ def run_ours(a):
         te = time.perf_counter()
         v_e2e = e2e_step()
         e2e_ms += (time.perf_counter() - te) * 1e3
-    e2e_ms_max, e2e_units = all_reduce_max_sum(e2e_ms, float(Rd.shape[0] * n_e2e), world, dev)
+    e2e_ms_max, e2e_units = all_reduce_max_sum(e2e_ms, float(Rd.shape[0] * n_e2e), world, rdev)
     if not blocks_mode and not (np.isfinite(v_e2e) and abs(v_e2e - st1["veff"]) <= 1e-5 * abs(st1["veff"])):
         raise RuntimeError("host-buffer evaluation disagrees with the device-buffer one: %r vs %r" % (v_e2e, st1["veff"]))
     if not np.isfinite(v_e2e):
@@ -513,6 +522,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--blocks-on-one-gpu", action="store_true",
                     help="--gpus 1 through the bead-block driver (one block = the whole path): exercises that code path")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="gloo: halos and reductions staged through host memory (needed when several ranks share a GPU)")
+    ap.add_argument("--all-ranks-on-one-gpu", action="store_true",
+                    help="every rank uses cuda:0: runs the N-rank code path on one GPU (functional check, not a scaling "
+                         "number; use with --dist-backend gloo -- NCCL needs one GPU per rank)")
     ap.add_argument("--parallelism", default="blocks", choices=["blocks", "replicas"],
                     help="--gpus N > 1: one path sharded by bead blocks with halo exchange (default), or independent replicas")
     a = ap.parse_args()

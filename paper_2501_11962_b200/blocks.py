@@ -47,12 +47,29 @@ def _wait(reqs):
         r.wait()
 
 
+class _Staged:
+    """A halo exchange that goes through host memory (host_staging): the requests, and the copy of the received host
+    tensor into the device tensor that has to follow their completion."""
+
+    def __init__(self, reqs, host, dev):
+        self.reqs, self.host, self.dev = reqs, host, dev
+
+    def wait(self):
+        _wait(self.reqs)
+        if self.dev is not None:
+            self.dev.copy_(self.host)
+
+
 class BlockPath:
     """One rank's share of a sharded evaluation.  rank/world default to the default process group's; world = 1 needs no
-    process group at all (the block is the whole path)."""
+    process group at all (the block is the whole path).
+    host_staging: device halos travel as host copies (send: device -> host, receive: host -> device) and the 8-byte
+    reduction runs on a host tensor, so that a process group without device support (gloo) can drive GPU engines -- the
+    functional multi-rank run on ONE GPU (bench.py --dist-backend gloo --all-ranks-on-one-gpu); slower, same results."""
 
     def __init__(self, engine, n_atoms, first_bead, n_beads, n_beads_path, rank=None, world=None, device="cpu",
-                 dtype=torch.float32, group=None):
+                 dtype=torch.float32, group=None, host_staging=False):
+        self.host_staging = bool(host_staging)
         self.engine = engine
         self.world = world if world is not None else (dist.get_world_size(group) if dist.is_initialized() else 1)
         self.rank = rank if rank is not None else (dist.get_rank(group) if dist.is_initialized() else 0)
@@ -64,22 +81,31 @@ class BlockPath:
         self.right = self.rank + 1 if self.has_right else None
         mk = lambda: torch.zeros((n_atoms, 3), dtype=dtype, device=device)
         self.R_right, self.keta_out, self.keta_left = mk(), mk(), mk()
-        self._vbuf = torch.zeros(1, dtype=torch.float64, device=device)
+        self._vbuf = torch.zeros(1, dtype=torch.float64, device="cpu" if self.host_staging else device)
+        self._h_recv = torch.zeros((n_atoms, 3), dtype=dtype) if self.host_staging else None
+
+    def _halo(self, send_to, send_tensor, recv_from, recv_tensor):
+        """Non-blocking exchange of one halo each way; returns something with .wait()."""
+        if not self.host_staging:
+            return _Staged(_exchange(send_to, send_tensor, recv_from, recv_tensor, self.group), None, None)
+        h_send = send_tensor.cpu() if send_to is not None else None     # synchronises this rank's stream: the halo is ready
+        reqs = _exchange(send_to, h_send, recv_from, self._h_recv, self.group)
+        return _Staged(reqs, self._h_recv, recv_tensor if recv_from is not None else None)
 
     def eval(self, R_block, grad_out=None, sync=True):
         """R_block [n_beads][Q][3] (this rank's beads).  Returns (V_eff of the WHOLE path, gradient of this block).
         sync=False: the assembly stays asynchronous and no V_eff is formed (returns (None, gradient)): a stepping loop needs
         the gradient only; read the energy when it is wanted with veff()."""
         # 1. right halo of the coordinates
-        _wait(_exchange(self.left, R_block[0].contiguous(), self.right, self.R_right, self.group))
+        self._halo(self.left, R_block[0].contiguous(), self.right, self.R_right).wait()
         # 2. pass 1
         self.engine.mop_block_pass1(R_block, self.R_right if self.has_right else None,
                                     self.keta_out if self.has_right else None)
         # 3. K eta halo in flight during pass 2
-        reqs = _exchange(self.right, self.keta_out, self.left, self.keta_left, self.group)
+        halo = self._halo(self.right, self.keta_out, self.left, self.keta_left)
         # 4. pass 2
         self.engine.mop_block_pass2(R_block)
-        _wait(reqs)
+        halo.wait()
         # 5. assembly and the 8-byte reduction
         if not sync:
             return self.engine.mop_block_assemble(self.keta_left if self.has_left else None, grad_out, sync=False)

@@ -180,3 +180,37 @@ def test_block_path_driver_single_rank(B, oracle):
     assert abs(v - v_ref) <= 1e-6 * abs(v_ref)
     H.assert_close(g.cpu().numpy(), g_ref, 1e-4)
     eng.close()
+
+
+@pytest.mark.parametrize("ranks,config,beads,port", [(4, 2, 4, 29561), (8, 4, 8, 29563)])
+def test_bench_block_arm_with_n_ranks_on_one_gpu(B, ranks, config, beads, port):
+    """The code path `bench.py --gpus N` takes, run with N real ranks before any multi-GPU box does: N processes (torchrun),
+    every one with its own bead-block context on cuda:0, the halos and the 8-byte reduction staged through host memory
+    under gloo (NCCL wants one GPU per rank).  Same partition, same BlockPath, the real engine.  FUNCTIONAL, not a scaling
+    number: the ranks share one GPU.  Rank 0's V_eff must be that of ONE context evaluating the same N x beads path --
+    to 1e-6 only, because every rank generates the path itself with the library's force, whose float atomics differ in the
+    last bits from process to process (a few coordinates round to the neighbouring FP32 value)."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(ranks), "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", str(ranks), "--config", str(config),
+           "--beads", str(beads), "--steps", "2", "--warmup", "3", "--dist-backend", "gloo", "--all-ranks-on-one-gpu",
+           "--no-cpu-baseline"]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=1500, cwd=root)
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    out = json.loads([l for l in r.stdout.splitlines() if l.startswith("{")][-1])
+    n_path = ranks * beads
+    assert out["n_gpus"] == ranks and "bead blocks: %d ranks x %d beads of one %d-bead path" % (ranks, beads, n_path) in \
+        out["config"]["parallelism"] and "not a scaling number" in out["config"]["parallelism"]
+    assert out["value"] > 0 and out["e2e"]["value"] > 0 and out["gpu_launches"] > 0
+    s = W.CONFIGS[config](seed=0, n_beads=n_path)
+    m1 = B.Mop(s, 1)
+    R = W.folded_path(s, n_path, lambda X: m1.mop_force_hvp(X)[0].double().cpu().numpy(), seed=0)
+    m1.close()
+    m = B.Mop(s, n_path)
+    v, _ = m.mop_eval_veff_grad(R, want_grad=False)
+    m.close()
+    assert abs(out["veff"] - v) <= 1e-6 * abs(v), (out["veff"], v)

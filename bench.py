@@ -38,7 +38,7 @@ FLOP_PER_PAIR_FORCE = 31.0
 FLOP_PER_PAIR_HVP = 55.0
 # The ncu capture of the dominant kernel (S5) on the bench workload, committed under profiles/: a two-column CSV
 # "metric,value" for one launch, written from the .ncu-rep by the command in profiles/r02_ncu_summary.md.
-NCU_METRICS_FILE = os.path.join("profiles", "r02_ncu_hvp_metrics.csv")
+NCU_METRICS_FILE = os.path.join("profiles", "r03_ncu_hvp_metrics.csv")
 
 
 def traffic_bytes_per_launch():
